@@ -1,0 +1,167 @@
+"""Pins for the oracle's voxel SDF, generated marching-cubes table and polygoniser (S14-S17).  CPU only."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import refbind as R
+from tests import meshutil as M
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _sp(h=0.0625):
+    return dict(box_min=(0.0, 0.0, 0.0), box_max=(1.0, 1.0, 1.0), h=h, rest_density=1000.0, mass=0.03,
+                stiffness=3.0, viscosity=0.1, gravity=(0.0, -9.81, 0.0), dt=1e-3, wall_damping=0.5)
+
+
+def _mp(G, origin=(0.0, 0.0, 0.0), spacing=None, R_=0.0625, rbar=0.03125, iso=0.0):
+    return dict(origin=origin, spacing=spacing if spacing is not None else 1.0 / (G - 1), n_point_per_axis=G,
+                radius=R_, particle_radius=rbar, iso=iso)
+
+
+def _corners(mp):
+    G = mp["n_point_per_axis"]
+    k, j, i = np.meshgrid(np.arange(G), np.arange(G), np.arange(G), indexing="ij")
+    o, s = np.float32(mp["origin"]), np.float32(mp["spacing"])
+    return np.stack([o[0] + i.astype(np.float32) * s, o[1] + j.astype(np.float32) * s,
+                     o[2] + k.astype(np.float32) * s], -1).reshape(-1, 3)
+
+
+def test_sdf_single_particle_is_a_distance():
+    # P:477 Eq. 48 with one neighbour: xbar = x1, so phi = |x - x1| - rbar inside R, and R - rbar outside (D:A-PHI0)
+    mp = _mp(24, origin=(0.4, 0.4, 0.4), spacing=0.008)
+    x1 = np.array([[0.4913, 0.5021, 0.4876, 0]], np.float32)
+    phi = R.voxel_sdf(_sp(), mp, x1)
+    d = np.linalg.norm(_corners(mp).astype(np.float64) - x1[0, :3].astype(np.float64), axis=1)
+    inside = d < 0.0625 * (1 - 1e-6)
+    outside = d > 0.0625 * (1 + 1e-6)
+    assert inside.sum() > 1000 and outside.sum() > 1000
+    assert np.allclose(phi[inside], d[inside] - 0.03125, atol=2e-7)
+    assert np.all(phi[outside] == np.float32(0.0625 - 0.03125))
+
+
+def test_sdf_symmetric_pair_and_brute_force():
+    mp = _mp(9, origin=(0.5, 0.5, 0.5), spacing=0.0)  # every corner at the same point
+    pts = np.array([[0.52, 0.5, 0.5, 0], [0.48, 0.5, 0.5, 0]], np.float32)
+    phi = R.voxel_sdf(_sp(), mp, pts)
+    assert np.allclose(phi, -0.03125, atol=1e-7)  # S1 = 0 -> phi = -rbar
+    from paper_2311_15088_b200 import workloads as W
+    cfg = W.config(1, scale=2)
+    mp = _mp(20, spacing=0.3 / 19)
+    a = R.voxel_sdf(cfg["sph"], mp, cfg["pos"])
+    b = R.voxel_sdf(cfg["sph"], mp, cfg["pos"], brute=True)
+    assert np.allclose(a, b, rtol=0, atol=1e-7)
+    assert (a < 0).any() and (a > 0).any()
+
+
+def test_table_worked_example_and_structure():
+    tri, ntri, edge = R.mc_table()
+    corners, edges = R.mc_numbering()
+    # only corner 3 below the isolevel -> cube_index 8 -> edge_table[8] = 0x80c -> edges 2, 3, 11
+    assert edge[8] == 0x80C and ntri[8] == 1 and sorted(tri[8][:3]) == [2, 3, 11] and tri[8][3] == -1
+    assert {e for e in range(12) if 3 in edges[e]} == {2, 3, 11}
+    assert ntri[0] == 0 and ntri[255] == 0 and edge[0] == 0 and edge[255] == 0
+    for cs in range(256):
+        below = [(cs >> n) & 1 for n in range(8)]
+        crossed = {e for e in range(12) if below[edges[e][0]] != below[edges[e][1]]}
+        used = {int(e) for e in tri[cs] if e >= 0}
+        assert used == crossed, cs                                  # cover all sign-changing edges, and only them
+        assert edge[cs] == sum(1 << e for e in crossed)
+        n = ntri[cs]
+        assert 0 <= n <= 5 and all(tri[cs][3 * n:] == -1) and all(tri[cs][:3 * n] >= 0)
+        assert edge[cs] == edge[255 - cs]                            # complement has the same crossed edges
+        # every triangle uses three distinct edges
+        for t in range(n):
+            assert len(set(tri[cs][3 * t:3 * t + 3])) == 3
+    # a single corner below gives one triangle around it; its complement too
+    for n in range(8):
+        assert ntri[1 << n] == 1 and ntri[255 - (1 << n)] == 1
+
+
+def test_table_matches_golden_counts():
+    # tests/golden/mc_ntri.txt is written by tests/golden/make_golden.py from the oracle AFTER the pins here passed
+    _, ntri, _ = R.mc_table()
+    gold = np.loadtxt(os.path.join(GOLDEN, "mc_ntri.txt"), dtype=np.int64, comments="#")
+    assert np.array_equal(gold.reshape(-1), ntri)
+
+
+def _closed_field(G, seed, smooth):
+    rng = np.random.default_rng(seed)
+    f = rng.standard_normal((G, G, G))
+    for _ in range(smooth):
+        f = (f + np.roll(f, 1, 0) + np.roll(f, 1, 1) + np.roll(f, 1, 2)) / 4.0
+    f = f - np.median(f)
+    f[0], f[-1], f[:, 0], f[:, -1], f[:, :, 0], f[:, :, -1] = (1.0,) * 6  # outside everywhere on the boundary
+    return f.astype(np.float32).reshape(-1)
+
+
+@pytest.mark.parametrize("seed,smooth", [(0, 0), (1, 0), (2, 1), (3, 3)])
+def test_random_fields_give_closed_consistently_oriented_meshes(seed, smooth):
+    # white noise exercises all 256 cases and every pair of face-adjacent cases, ambiguous faces included:
+    # crack-free <=> every mesh edge is shared by exactly two triangles, traversed once in each direction
+    G = 14
+    phi = _closed_field(G, seed, smooth)
+    mp = _mp(G)
+    tris, nt, cases = R.mc_polygonise(mp, phi, want_cases=True)
+    assert nt == len(tris) and nt > 100
+    if smooth == 0:
+        assert len(np.unique(cases)) > 250
+    ids, _ = M.weld(tris)
+    _, ok, degenerate = M.edge_stats(ids)
+    assert degenerate == 0
+    assert ok
+    # triangle count = sum over cubes of ntri[case]; order = cube-major (D:A-APPEND)
+    _, ntri, _ = R.mc_table()
+    assert nt == int(ntri[cases].sum())
+    # volume enclosed (normals point to the >= iso side) is positive and below the grid volume
+    _, vol, _ = M.area_volume(tris)
+    assert 0 < vol < 1.0
+
+
+@pytest.mark.parametrize("G,tol_area", [(32, 0.01), (64, 0.003)])
+def test_sphere_isosurface(G, tol_area):
+    # north_star pin: watertight sphere, area close to 4 pi r^2 (r = 10 voxels at G = 32)
+    mp = _mp(G)
+    c = np.array([0.5, 0.5, 0.5]) + 0.37 / (G - 1)
+    r = 10.0 / 31.0
+    x = _corners(mp).astype(np.float64)
+    phi = (np.linalg.norm(x - c, axis=1) - r).astype(np.float32)
+    tris, nt, _ = R.mc_polygonise(mp, phi)
+    ids, nv = M.weld(tris)
+    ne, ok, degenerate = M.edge_stats(ids)
+    assert ok and degenerate == 0
+    assert nv - ne + nt == 2                                     # Euler characteristic of a sphere
+    area, vol, normals = M.area_volume(tris)
+    assert abs(area / (4 * math.pi * r * r) - 1) < tol_area
+    assert abs(vol / (4 / 3 * math.pi * r ** 3) - 1) < 2 * tol_area
+    centroid = tris.astype(np.float64).mean(1)
+    assert np.all(np.einsum("ij,ij->i", normals, centroid - c) > 0)  # outward
+    # vertices lie on the sphere to O(spacing^2) (Eq. 51 linear interpolation)
+    v = tris.reshape(-1, 3).astype(np.float64)
+    assert np.abs(np.linalg.norm(v - c, axis=1) - r).max() < 0.6 * mp["spacing"] ** 2 / r + 1e-6
+
+
+def test_capacity_is_respected():
+    mp = _mp(16)
+    x = _corners(mp).astype(np.float64)
+    phi = (np.linalg.norm(x - 0.5, axis=1) - 0.3).astype(np.float32)
+    full, nt, _ = R.mc_polygonise(mp, phi)
+    part, nt2, _ = R.mc_polygonise(mp, phi, capacity=nt // 2)
+    assert nt2 == nt and len(part) == nt // 2 and np.array_equal(part, full[:nt // 2])
+
+
+def test_single_particle_through_sdf_and_mc_gives_sphere_of_radius_rbar():
+    h = 0.0625
+    G = 40
+    mp = _mp(G, origin=(0.45, 0.45, 0.45), spacing=0.1 / (G - 1))
+    x1 = np.array([[0.5003, 0.4991, 0.5007, 0]], np.float32)
+    phi = R.voxel_sdf(_sp(h), mp, x1)
+    tris, nt, _ = R.mc_polygonise(mp, phi)
+    ids, nv = M.weld(tris)
+    ne, ok, _ = M.edge_stats(ids)
+    assert ok and nv - ne + nt == 2
+    v = tris.reshape(-1, 3).astype(np.float64)
+    # linear interpolation (Eq. 51) of a distance function along an edge errs by at most spacing^2 / (8 r)
+    assert np.abs(np.linalg.norm(v - x1[0, :3], axis=1) - 0.5 * h).max() < 1.1 * mp["spacing"] ** 2 / (8 * 0.5 * h)
