@@ -1,0 +1,144 @@
+/* sphboid.h -- C ABI of libsphboid: the per-frame particle pipeline of arXiv 2311.15088
+ * ("A GPU-based Hydrodynamic Simulator with Boid Interactions") as hand-written CUDA for sm_100a.
+ *
+ * Citations: "P:n" = line n of the paper text; "D:X" = reading X in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Every array argument is a DEVICE pointer unless its name ends in _host or the comment says
+ *     "host".  Particle / boid state is SoA float4: pos[i] = (x,y,z,-), vel[i] = (vx,vy,vz,-),
+ *     16-byte aligned; the 4th lane is carried through untouched.
+ *   - The caller owns every state and output array.  The library owns only the scratch it sized in
+ *     sph_create from the max_* fields (cell keys, histogram, starts, permutation, sorted copies,
+ *     densities, boid grid, phi, scan state).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls only
+ *     enqueue work on it; the single host synchronisation is the optional triangle-count read in
+ *     mc_extract / mc_polygonise (pass n_tris_host = NULL to skip it) and the *_host entry points.
+ *   - Outputs are in the CALLER'S particle order; the cell-sorted copy is internal.
+ *   - Every function returns SPH_OK (0) or a negative sph_status; nothing throws or aborts.
+ *     sph_last_error(ctx) gives a message for the last failure on that context.
+ *   - There is no CPU fallback: without a CUDA device sph_create fails with SPH_E_CUDA.
+ */
+#ifndef SPHBOID_H
+#define SPHBOID_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sph_ctx sph_ctx; /* opaque, library-owned */
+
+typedef enum {
+  SPH_OK = 0,
+  SPH_E_INVALID = -1,    /* null / misaligned pointer, n > max, h <= 0, empty box, bad params */
+  SPH_E_CAPACITY = -2,   /* triangle buffer too small: nothing past capacity written, count still returned */
+  SPH_E_STALE_GRID = -3, /* call needs a grid / step state that is not current */
+  SPH_E_CUDA = -4,       /* CUDA runtime error, see sph_last_error */
+  SPH_E_UNIMPL = -5
+} sph_status;
+
+/* SPH parameters.  bound = {min,max} and cell size d (Eq. 47); h, rho0, k, mu
+ * (Eq. 27-45); Euler-Cromer step and damped walls. */
+typedef struct {
+  float box_min[3], box_max[3];
+  float h;                                   /* smoothing length == grid cell size d (D:A-CELLSIZE) */
+  float rest_density, mass, stiffness, viscosity; /* rho0, m, k (bulk_modulus), mu */
+  float gravity[3], dt, wall_damping;
+  uint32_t max_particles, max_boids, max_mc_points_per_axis; /* scratch sizing */
+} sph_params;
+
+/* Boid parameters: separation inside protect_range, alignment + cohesion inside
+ * visible_range, weights "sep", "mat", "cen"; speed limits, edge rule (D:C-EDGE); fluid->boid gain
+ * sph_factor; boid->fluid radius R_p and gain (D:C-COUPLE); Boid Space. */
+typedef struct {
+  float protect_range, visible_range;
+  float w_sep, w_ali, w_coh;
+  float min_speed, max_speed, edge_turn;
+  float sph_factor;
+  float push_radius, w_push;
+  float space_min[3], space_max[3];
+} boid_params;
+
+/* Surface pass (P:475-517 voxel density, P:531-562 marching cubes).
+ * corner(i,j,k) = origin + (i,j,k)*spacing, linear index i + G*(j + G*k); (G-1)^3 cubes. */
+typedef struct {
+  float origin[3], spacing;
+  uint32_t n_point_per_axis;                 /* G */
+  float radius, particle_radius, iso;        /* R, r-bar, isolevel */
+} mc_params;
+
+/* Create a context on CUDA device `device`, allocating all scratch.  *out is NULL on failure. */
+int sph_create(sph_ctx** out, const sph_params* p, int device);
+int sph_destroy(sph_ctx* ctx);
+const char* sph_last_error(const sph_ctx* ctx); /* host string, valid until the next call on ctx */
+
+/* Grid dimensions dim = max(1, ceil((max-min)/h)) (D:A-DIMS); returns C = product. */
+uint32_t sph_grid_dims(const sph_ctx* ctx, uint32_t dims_out[3] /* host */);
+
+/* S1-S5: uniform-grid neighbour structure.
+ *   key = hash(get_cell(p)), clamped cells (D:A-CLAMPCELL); histogram; device-wide exclusive scan;
+ *   counting-sort scatter with the canonical within-cell order = ascending particle id (D:A-SORT);
+ *   cell-sorted copies of pos (and of vel when given) kept in the context.
+ * pos[n]; vel may be NULL (mc_extract needs positions only).
+ * Optional outputs (NULL to skip): cell_of_particle[n], perm[n] (sorted slot -> particle id),
+ * cell_start[C+1] (exclusive starts, cell_start[C] = n). */
+int sph_build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, void* stream,
+                   uint32_t* cell_of_particle, uint32_t* perm, uint32_t* cell_start);
+
+/* S6-S10: one SPH step, in place on pos / vel.
+ *   density rho_i = sum_j m W_poly6 (self included), neighbour count;
+ *   f_i = sum_j Listing-3 pair term; boids push the fluid (D:C-COUPLE); a_i = f_i/rho_i + g (D:A-RHO);
+ *   v += a dt, x += v dt (Euler-Cromer), damped wall clamp (D:A-WALL).
+ * Builds the grid itself unless the last sph_build_grid was on this (pos, vel, n).
+ * bpos / bvel [n_boid] are the step-start boids (not modified); bp may be NULL iff n_boid == 0.
+ * Optional outputs in caller order (NULL to skip): density[n], accel[n] (float4, total a_i),
+ * ncount[n], touched[n] (number of boids inside the push radius). */
+int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, const void* bvel,
+             uint32_t n_boid, const boid_params* bp /* host */, void* stream, float* density, void* accel,
+             uint32_t* ncount, uint32_t* touched);
+
+/* S11-S13: one boid step, in place on bpos / bvel.
+ *   separation / alignment / cohesion on step-start state (D:C-JACOBI), fluid force on the boid from the
+ *   step-start fluid state retained by the sph_step of the same frame (D:C-COUPLE), edge rule, speed
+ *   clamp, position update.
+ * Must follow sph_step called with these same (unmodified) bpos / bvel; otherwise SPH_E_STALE_GRID.
+ * Optional dv_parts[n_boid*4] float4: the sep, ali, coh, fluid velocity increments per boid. */
+int boid_step(sph_ctx* ctx, const boid_params* bp /* host */, void* bpos, void* bvel, uint32_t n_boid,
+              void* stream, void* dv_parts);
+
+/* S14: voxel signed distance phi(x) = |x - xbar| - rbar, xbar the kernel-weighted mean neighbour position
+ * (Eq. 48-50, Listing 9; D:A-PHI, D:A-PHI0).  Needs a current grid (sph_build_grid on the
+ * positions to mesh) else SPH_E_STALE_GRID.  phi[G^3]. */
+int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, float* phi);
+
+/* S15-S17: marching cubes on a given phi[G^3] (Listing 10-11, Eq. 51): case per cube,
+ * triangle count, device-wide exclusive scan, ordered emit (cube-major, then table order; D:A-APPEND).
+ * tris = tri_capacity * 9 floats (3 vertices x xyz).  *n_tris_host (host, optional) gets the REQUIRED
+ * count; if it exceeds tri_capacity the return value is SPH_E_CAPACITY and nothing past capacity is written.
+ * n_tris_dev (device, optional) receives the same count without a host sync. */
+int mc_polygonise(sph_ctx* ctx, const mc_params* mp /* host */, const float* phi, void* stream, float* tris,
+                  uint32_t tri_capacity, uint32_t* n_tris_host, uint32_t* n_tris_dev);
+
+/* S14-S17 in one call: phi may be NULL (library scratch is used) or a G^3 buffer that receives phi. */
+int mc_extract(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, float* phi, float* tris,
+               uint32_t tri_capacity, uint32_t* n_tris_host);
+
+/* End-to-end frame with HOST buffers (pinned or pageable): copies pos/vel/bpos/bvel to the device, runs
+ * `steps` frames of sph_build_grid + sph_step + boid_step, optionally one surface pass on the final
+ * positions (mp != NULL), copies the state (and triangles) back and synchronises.
+ * tris_host may be NULL when mp is NULL. */
+int sph_simulate_host(sph_ctx* ctx, float* pos_host, float* vel_host, uint32_t n, float* bpos_host,
+                      float* bvel_host, uint32_t n_boid, const boid_params* bp, uint32_t steps,
+                      const mc_params* mp, float* tris_host, uint32_t tri_capacity, uint32_t* n_tris_host);
+
+/* The marching-cubes table the library uses (generated, D:M-TABLE): tri[256*16] edge ids, -1 terminated. */
+void sph_mc_table(int8_t* tri_host, uint8_t* ntri_host);
+
+/* Number of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
+uint64_t sph_launch_count(const sph_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

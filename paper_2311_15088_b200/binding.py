@@ -1,0 +1,215 @@
+"""ctypes binding of libsphboid.so -- same names as include/sphboid.h, argument marshalling only.
+
+Device arrays are torch CUDA tensors (PyTorch supplies device memory and streams, nothing else): float32
+(n,4) for pos / vel / bpos / bvel / accel, uint32-as-int32 for index outputs.  Every step of the path runs
+in the library's CUDA kernels; there is NO CPU fallback -- a missing library or device raises.
+"""
+import ctypes as C
+import os
+
+_f = C.c_float
+_u32 = C.c_uint32
+_vp = C.c_void_p
+
+SPH_OK, SPH_E_INVALID, SPH_E_CAPACITY, SPH_E_STALE_GRID, SPH_E_CUDA, SPH_E_UNIMPL = 0, -1, -2, -3, -4, -5
+
+
+class SphParams(C.Structure):
+    _fields_ = [("box_min", _f * 3), ("box_max", _f * 3), ("h", _f), ("rest_density", _f), ("mass", _f),
+                ("stiffness", _f), ("viscosity", _f), ("gravity", _f * 3), ("dt", _f), ("wall_damping", _f),
+                ("max_particles", _u32), ("max_boids", _u32), ("max_mc_points_per_axis", _u32)]
+
+
+class BoidParams(C.Structure):
+    _fields_ = [("protect_range", _f), ("visible_range", _f), ("w_sep", _f), ("w_ali", _f), ("w_coh", _f),
+                ("min_speed", _f), ("max_speed", _f), ("edge_turn", _f), ("sph_factor", _f), ("push_radius", _f),
+                ("w_push", _f), ("space_min", _f * 3), ("space_max", _f * 3)]
+
+
+class McParams(C.Structure):
+    _fields_ = [("origin", _f * 3), ("spacing", _f), ("n_point_per_axis", _u32), ("radius", _f),
+                ("particle_radius", _f), ("iso", _f)]
+
+
+class SphError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libsphboid error %d: %s" % (code, msg))
+        self.code = code
+
+
+def _fill(struct, d):
+    if isinstance(d, struct):
+        return d
+    s = struct()
+    for name, ctype in struct._fields_:
+        if name not in d:
+            continue
+        v = d[name]
+        if hasattr(ctype, "_length_"):
+            setattr(s, name, ctype(*[float(x) for x in v]))
+        else:
+            setattr(s, name, v)
+    return s
+
+
+LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libsphboid.so")
+_lib = None
+
+
+def lib():
+    """Load libsphboid.so (built in-tree by paper_2311_15088_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libsphboid.so is not built: run `python -m paper_2311_15088_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.sph_create.argtypes = [C.POINTER(_vp), _vp, C.c_int]
+        L.sph_destroy.argtypes = [_vp]
+        L.sph_last_error.argtypes = [_vp]
+        L.sph_last_error.restype = C.c_char_p
+        L.sph_grid_dims.argtypes = [_vp, _vp]
+        L.sph_grid_dims.restype = _u32
+        L.sph_build_grid.argtypes = [_vp, _vp, _vp, _u32, _vp, _vp, _vp, _vp]
+        L.sph_step.argtypes = [_vp, _vp, _vp, _u32, _vp, _vp, _u32, _vp, _vp, _vp, _vp, _vp, _vp]
+        L.boid_step.argtypes = [_vp, _vp, _vp, _vp, _u32, _vp, _vp]
+        L.mc_voxel_sdf.argtypes = [_vp, _vp, _vp, _vp]
+        L.mc_polygonise.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp, _vp]
+        L.mc_extract.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp]
+        L.sph_simulate_host.argtypes = [_vp, _vp, _vp, _u32, _vp, _vp, _u32, _vp, _u32, _vp, _vp, _u32, _vp]
+        L.sph_mc_table.argtypes = [_vp, _vp]
+        L.sph_mc_table.restype = None
+        L.sph_launch_count.argtypes = [_vp]
+        L.sph_launch_count.restype = C.c_uint64
+        _lib = L
+    return _lib
+
+
+EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
+           "mc_voxel_sdf", "mc_polygonise", "mc_extract", "sph_simulate_host", "sph_mc_table", "sph_launch_count"]
+
+
+def _ptr(t):
+    """Device pointer of a torch CUDA tensor (or None)."""
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "expected a contiguous CUDA tensor"
+    return _vp(t.data_ptr())
+
+
+def _hptr(a):
+    """Host pointer of a numpy array or CPU torch tensor (or None)."""
+    if a is None:
+        return None
+    if hasattr(a, "data_ptr"):
+        assert not a.is_cuda and a.is_contiguous()
+        return _vp(a.data_ptr())
+    assert a.flags["C_CONTIGUOUS"]
+    return _vp(a.ctypes.data)
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    elif hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    return _vp(stream)
+
+
+def _check(ctx, rc, allow=()):
+    if rc != SPH_OK and rc not in allow:
+        raise SphError(rc, lib().sph_last_error(ctx).decode() if ctx else "no context")
+    return rc
+
+
+def sph_create(params, max_particles, max_boids=0, max_mc_points_per_axis=0, device=0):
+    p = _fill(SphParams, dict(params, max_particles=max_particles, max_boids=max_boids,
+                              max_mc_points_per_axis=max_mc_points_per_axis))
+    h = _vp()
+    rc = lib().sph_create(C.byref(h), C.byref(p), device)
+    if rc != SPH_OK:
+        raise SphError(rc, "sph_create failed (no CUDA device, bad parameters or out of memory)")
+    return h
+
+
+def sph_destroy(ctx):
+    lib().sph_destroy(ctx)
+
+
+def sph_grid_dims(ctx):
+    dims = (_u32 * 3)()
+    c = lib().sph_grid_dims(ctx, dims)
+    return tuple(dims), int(c)
+
+
+def sph_launch_count(ctx):
+    return int(lib().sph_launch_count(ctx))
+
+
+def sph_mc_table():
+    import numpy as np
+    tri = np.zeros((256, 16), np.int8)
+    ntri = np.zeros(256, np.uint8)
+    lib().sph_mc_table(_hptr(tri), _hptr(ntri))
+    return tri, ntri
+
+
+def sph_build_grid(ctx, pos, vel=None, stream=None, cell_of_particle=None, perm=None, cell_start=None):
+    n = 0 if pos is None else pos.shape[0]
+    return _check(ctx, lib().sph_build_grid(ctx, _ptr(pos), _ptr(vel), n, _stream(stream), _ptr(cell_of_particle),
+                                            _ptr(perm), _ptr(cell_start)))
+
+
+def sph_step(ctx, pos, vel, bpos=None, bvel=None, boid=None, stream=None, density=None, accel=None, ncount=None,
+             touched=None):
+    nb = 0 if bpos is None else bpos.shape[0]
+    bp = _fill(BoidParams, boid) if nb else None
+    return _check(ctx, lib().sph_step(ctx, _ptr(pos), _ptr(vel), pos.shape[0], _ptr(bpos) if nb else None,
+                                      _ptr(bvel) if nb else None, nb, C.byref(bp) if nb else None, _stream(stream),
+                                      _ptr(density), _ptr(accel), _ptr(ncount), _ptr(touched)))
+
+
+def boid_step(ctx, boid, bpos, bvel, stream=None, dv_parts=None):
+    bp = _fill(BoidParams, boid)
+    return _check(ctx, lib().boid_step(ctx, C.byref(bp), _ptr(bpos), _ptr(bvel), bpos.shape[0], _stream(stream),
+                                       _ptr(dv_parts)))
+
+
+def mc_voxel_sdf(ctx, mc, phi, stream=None):
+    m = _fill(McParams, mc)
+    return _check(ctx, lib().mc_voxel_sdf(ctx, C.byref(m), _stream(stream), _ptr(phi)))
+
+
+def mc_polygonise(ctx, mc, phi, tris, stream=None, sync=True, n_tris_dev=None):
+    """Returns the required triangle count (int) when sync, else None.  tris: (capacity, 3, 3) float32 CUDA."""
+    m = _fill(McParams, mc)
+    nt = _u32(0)
+    cap = 0 if tris is None else tris.shape[0]
+    rc = lib().mc_polygonise(ctx, C.byref(m), _ptr(phi), _stream(stream), _ptr(tris), cap,
+                             C.byref(nt) if sync else None, _ptr(n_tris_dev))
+    _check(ctx, rc, allow=(SPH_E_CAPACITY,))
+    return int(nt.value) if sync else None
+
+
+def mc_extract(ctx, mc, tris, phi=None, stream=None, sync=True):
+    m = _fill(McParams, mc)
+    nt = _u32(0)
+    cap = 0 if tris is None else tris.shape[0]
+    rc = lib().mc_extract(ctx, C.byref(m), _stream(stream), _ptr(phi), _ptr(tris), cap, C.byref(nt) if sync else None)
+    _check(ctx, rc, allow=(SPH_E_CAPACITY,))
+    return int(nt.value) if sync else None
+
+
+def sph_simulate_host(ctx, pos, vel, bpos=None, bvel=None, boid=None, steps=1, mc=None, tris=None):
+    """HOST arrays (numpy / pinned CPU tensors) in and out; returns the required triangle count."""
+    nb = 0 if bpos is None else bpos.shape[0]
+    bp = _fill(BoidParams, boid) if nb else None
+    m = _fill(McParams, mc) if mc is not None else None
+    nt = _u32(0)
+    cap = 0 if tris is None else tris.shape[0]
+    rc = lib().sph_simulate_host(ctx, _hptr(pos), _hptr(vel), pos.shape[0], _hptr(bpos) if nb else None,
+                                 _hptr(bvel) if nb else None, nb, C.byref(bp) if nb else None, steps,
+                                 C.byref(m) if m is not None else None, _hptr(tris), cap, C.byref(nt))
+    _check(ctx, rc, allow=(SPH_E_CAPACITY,))
+    return int(nt.value)

@@ -1,0 +1,424 @@
+// api.cu -- the C ABI of libsphboid (include/sphboid.h): context, scratch, argument checks, sequencing.
+#include "../../include/sphboid.h"
+
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "kernels.h"
+
+using namespace sphb;
+
+struct sph_ctx {
+  int device;
+  sph_params p;
+  SphConst sc;
+  GridBuf pg;   // particle grid
+  GridBuf bg;   // boid grid
+  uint32_t boid_cells_cap;
+  float* rhoS;
+  float* rho_bS;
+  float* phi;   // [Gmax^3]
+  uint32_t* n_tris_dev;
+  ScanState scan;
+  uint32_t max_tiles;
+  // sequencing
+  const void* grid_pos;
+  const void* grid_vel;
+  uint32_t grid_n;
+  bool grid_fresh;       // pg holds a grid of (grid_pos, grid_n) and positions have not moved since
+  bool step_state;       // pg/rhoS hold the step-start state of the last sph_step
+  BoidConst bc;
+  bool boid_state;       // bg/rho_bS hold the boids given to the last sph_step
+  const void* boid_pos;
+  uint32_t boid_n;
+  uint64_t launches;
+  char err[256];
+  // staging for the *_host entry point
+  float4 *h_pos, *h_vel, *h_bpos, *h_bvel;
+  float* h_tris;
+  uint32_t h_tris_cap;
+};
+
+namespace {
+
+int fail(sph_ctx* c, int code, const char* msg) {
+  if (c) snprintf(c->err, sizeof(c->err), "%s", msg);
+  return code;
+}
+
+int cuda_fail(sph_ctx* c, cudaError_t e, const char* where) {
+  if (c) snprintf(c->err, sizeof(c->err), "%s: %s", where, cudaGetErrorString(e));
+  return SPH_E_CUDA;
+}
+
+#define CK(call)                                           \
+  do {                                                     \
+    cudaError_t e_ = (call);                               \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); \
+  } while (0)
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// D:A-DIMS: dim = max(1, ceil((hi - lo)/cell)) in host double.
+bool make_grid(GridDesc& g, const float* lo, const float* hi, float cell) {
+  if (!(cell > 0.0f)) return false;
+  g.cell = cell;
+  uint64_t C = 1;
+  for (int a = 0; a < 3; ++a) {
+    if (!(hi[a] > lo[a])) return false;
+    g.lo[a] = lo[a];
+    double d = ceil(((double)hi[a] - (double)lo[a]) / (double)cell);
+    if (!(d >= 1.0)) d = 1.0;
+    if (d > 65535.0) return false;
+    g.dim[a] = (int)d;
+    C *= (uint64_t)g.dim[a];
+  }
+  if (C > (1ull << 30)) return false;
+  g.C = (uint32_t)C;
+  return true;
+}
+
+int alloc_grid(sph_ctx* ctx, GridBuf& b, uint32_t n, uint32_t C) {
+  const size_t nn = std::max<uint32_t>(n, 1);
+  CK(cudaMalloc(&b.key, nn * 4));
+  CK(cudaMalloc(&b.rank, nn * 4));
+  CK(cudaMalloc(&b.count, ((size_t)C + 8) * 4));
+  CK(cudaMalloc(&b.start, ((size_t)C + 9) * 4));
+  CK(cudaMalloc(&b.slot_id, nn * 4));
+  CK(cudaMalloc(&b.perm, nn * 4));
+  CK(cudaMalloc(&b.posS, nn * 16));
+  CK(cudaMalloc(&b.velS, nn * 16));
+  CK(cudaMemset(b.count, 0, ((size_t)C + 8) * 4));
+  CK(cudaMemset(b.start, 0, ((size_t)C + 9) * 4));
+  return SPH_OK;
+}
+
+void free_grid(GridBuf& b) {
+  cudaFree(b.key), cudaFree(b.rank), cudaFree(b.count), cudaFree(b.start);
+  cudaFree(b.slot_id), cudaFree(b.perm), cudaFree(b.posS), cudaFree(b.velS);
+  memset(&b, 0, sizeof(b));
+}
+
+int set_boid_params(sph_ctx* ctx, const boid_params* bp) {
+  if (!bp) return fail(ctx, SPH_E_INVALID, "boid_params is NULL");
+  BoidConst& bc = ctx->bc;
+  float cell = std::max(bp->visible_range, std::max(bp->protect_range, bp->push_radius));  // D:C-BGRID
+  if (!(cell > 0.0f) || !(bp->push_radius > 0.0f) || !(bp->visible_range > 0.0f) || !(bp->protect_range > 0.0f))
+    return fail(ctx, SPH_E_INVALID, "boid ranges must be positive");
+  GridDesc g;
+  if (!make_grid(g, bp->space_min, bp->space_max, cell)) return fail(ctx, SPH_E_INVALID, "bad Boid Space");
+  if (g.C > ctx->boid_cells_cap) {
+    // re-size the boid grid's cell arrays (host-side decision, rare: only when the ranges shrink)
+    cudaFree(ctx->bg.count), cudaFree(ctx->bg.start);
+    CK(cudaMalloc(&ctx->bg.count, ((size_t)g.C + 8) * 4));
+    CK(cudaMalloc(&ctx->bg.start, ((size_t)g.C + 9) * 4));
+    CK(cudaMemset(ctx->bg.count, 0, ((size_t)g.C + 8) * 4));
+    ctx->boid_cells_cap = g.C;
+    const uint32_t tiles = grid_scan_tiles(g.C);
+    if (tiles > ctx->max_tiles) {
+      cudaFree(ctx->scan.status);
+      CK(cudaMalloc(&ctx->scan.status, (size_t)tiles * 8));
+      CK(cudaMemset(ctx->scan.status, 0, (size_t)tiles * 8));
+      ctx->max_tiles = tiles;
+    }
+  }
+  bc.grid = g;
+  bc.protect = bp->protect_range, bc.visible = bp->visible_range;
+  bc.prot2 = bp->protect_range * bp->protect_range;
+  bc.vis2 = bp->visible_range * bp->visible_range;
+  bc.w_sep = bp->w_sep, bc.w_ali = bp->w_ali, bc.w_coh = bp->w_coh;
+  bc.min_speed = bp->min_speed, bc.max_speed = bp->max_speed, bc.edge_turn = bp->edge_turn;
+  bc.sph_factor = bp->sph_factor, bc.push_radius = bp->push_radius, bc.w_push = bp->w_push;
+  for (int a = 0; a < 3; ++a) bc.space_min[a] = bp->space_min[a], bc.space_max[a] = bp->space_max[a];
+  int r = (int)ceil((double)bp->push_radius / (double)ctx->p.h);
+  bc.reach_push = r < 1 ? 1 : r;
+  return SPH_OK;
+}
+
+int make_mc(sph_ctx* ctx, const mc_params* mp, McConst& m) {
+  if (!mp) return fail(ctx, SPH_E_INVALID, "mc_params is NULL");
+  if (mp->n_point_per_axis > ctx->p.max_mc_points_per_axis)
+    return fail(ctx, SPH_E_INVALID, "n_point_per_axis exceeds max_mc_points_per_axis");
+  if (!(mp->radius > 0.0f)) return fail(ctx, SPH_E_INVALID, "mc radius must be positive");
+  for (int a = 0; a < 3; ++a) m.origin[a] = mp->origin[a];
+  m.spacing = mp->spacing;
+  m.G = mp->n_point_per_axis;
+  m.R = mp->radius;
+  m.R2 = mp->radius * mp->radius;
+  m.rbar = mp->particle_radius;
+  m.iso = mp->iso;
+  int r = (int)ceil((double)mp->radius / (double)ctx->p.h);  // D:A-R
+  m.reach = r < 1 ? 1 : r;
+  return SPH_OK;
+}
+
+int build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, cudaStream_t s) {
+  launch_build_grid(ctx->sc.grid, ctx->pg, (const float4*)pos, (const float4*)vel, n, ctx->scan, s, &ctx->launches);
+  ctx->grid_pos = pos;
+  ctx->grid_vel = vel;
+  ctx->grid_n = n;
+  ctx->grid_fresh = true;
+  ctx->step_state = false;
+  return SPH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sph_create(sph_ctx** out, const sph_params* p, int device) {
+  if (!out) return SPH_E_INVALID;
+  *out = nullptr;
+  if (!p) return SPH_E_INVALID;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return SPH_E_CUDA;
+  sph_ctx* ctx = new (std::nothrow) sph_ctx();
+  if (!ctx) return SPH_E_CUDA;
+  memset(ctx, 0, sizeof(*ctx));
+  ctx->device = device;
+  ctx->p = *p;
+  SphConst& sc = ctx->sc;
+  if (!make_grid(sc.grid, p->box_min, p->box_max, p->h) || !(p->mass > 0.0f) || !(p->rest_density > 0.0f)) {
+    delete ctx;
+    return SPH_E_INVALID;
+  }
+  sc.h = p->h;
+  sc.h2 = p->h * p->h;
+  sc.mass = p->mass, sc.rho0 = p->rest_density, sc.stiffness = p->stiffness, sc.viscosity = p->viscosity;
+  sc.mass_c6 = (float)((double)p->mass * 315.0 / (64.0 * M_PI * pow((double)p->h, 9.0)));
+  for (int a = 0; a < 3; ++a)
+    sc.gravity[a] = p->gravity[a], sc.box_min[a] = p->box_min[a], sc.box_max[a] = p->box_max[a];
+  sc.dt = p->dt, sc.damp = p->wall_damping;
+
+  auto bail = [&](int code) {
+    sph_destroy(ctx);
+    return code;
+  };
+  if (cudaSetDevice(device) != cudaSuccess) return bail(SPH_E_CUDA);
+  if (alloc_grid(ctx, ctx->pg, p->max_particles, sc.grid.C) != SPH_OK) return bail(SPH_E_CUDA);
+  ctx->boid_cells_cap = 1u << 15;
+  if (alloc_grid(ctx, ctx->bg, p->max_boids, ctx->boid_cells_cap) != SPH_OK) return bail(SPH_E_CUDA);
+  const size_t nn = std::max<uint32_t>(p->max_particles, 1), nb = std::max<uint32_t>(p->max_boids, 1);
+  const size_t G = p->max_mc_points_per_axis;
+  if (cudaMalloc(&ctx->rhoS, nn * 4) != cudaSuccess || cudaMalloc(&ctx->rho_bS, nb * 4) != cudaSuccess ||
+      cudaMalloc(&ctx->phi, std::max<size_t>(G * G * G, 1) * 4) != cudaSuccess ||
+      cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess || cudaMalloc(&ctx->scan.ticket, 4) != cudaSuccess)
+    return bail(SPH_E_CUDA);
+  ctx->max_tiles = std::max(std::max(grid_scan_tiles(sc.grid.C), grid_scan_tiles(ctx->boid_cells_cap)),
+                            std::max(mc_num_tiles((uint32_t)G), 1u));
+  if (cudaMalloc(&ctx->scan.status, (size_t)ctx->max_tiles * 8) != cudaSuccess) return bail(SPH_E_CUDA);
+  cudaMemset(ctx->scan.status, 0, (size_t)ctx->max_tiles * 8);
+  cudaMemset(ctx->scan.ticket, 0, 4);
+  cudaMemset(ctx->n_tris_dev, 0, 4);
+  ctx->scan.ticket_base = 0;
+  ctx->scan.epoch = 0;
+  upload_mc_tables();
+  if (cudaDeviceSynchronize() != cudaSuccess) return bail(SPH_E_CUDA);
+  *out = ctx;
+  return SPH_OK;
+}
+
+int sph_destroy(sph_ctx* ctx) {
+  if (!ctx) return SPH_OK;
+  cudaSetDevice(ctx->device);
+  free_grid(ctx->pg);
+  free_grid(ctx->bg);
+  cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->n_tris_dev);
+  cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket);
+  cudaFree(ctx->h_pos), cudaFree(ctx->h_vel), cudaFree(ctx->h_bpos), cudaFree(ctx->h_bvel), cudaFree(ctx->h_tris);
+  delete ctx;
+  return SPH_OK;
+}
+
+const char* sph_last_error(const sph_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+uint32_t sph_grid_dims(const sph_ctx* ctx, uint32_t dims_out[3]) {
+  if (!ctx) return 0;
+  if (dims_out)
+    for (int a = 0; a < 3; ++a) dims_out[a] = (uint32_t)ctx->sc.grid.dim[a];
+  return ctx->sc.grid.C;
+}
+
+uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+void sph_mc_table(int8_t* tri_host, uint8_t* ntri_host) { mc_table_host(tri_host, ntri_host); }
+
+int sph_build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, void* stream,
+                   uint32_t* cell_of_particle, uint32_t* perm, uint32_t* cell_start) {
+  if (!ctx) return SPH_E_INVALID;
+  if (n > ctx->p.max_particles) return fail(ctx, SPH_E_INVALID, "n exceeds max_particles");
+  if (n > 0 && (!pos || !aligned16(pos) || !aligned16(vel)))
+    return fail(ctx, SPH_E_INVALID, "pos/vel must be 16-byte aligned device pointers");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  build_grid(ctx, pos, vel, n, s);
+  if (cell_of_particle && n) CK(cudaMemcpyAsync(cell_of_particle, ctx->pg.key, (size_t)n * 4, cudaMemcpyDeviceToDevice, s));
+  if (perm && n) CK(cudaMemcpyAsync(perm, ctx->pg.perm, (size_t)n * 4, cudaMemcpyDeviceToDevice, s));
+  if (cell_start)
+    CK(cudaMemcpyAsync(cell_start, ctx->pg.start, ((size_t)ctx->sc.grid.C + 1) * 4, cudaMemcpyDeviceToDevice, s));
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, const void* bvel, uint32_t n_boid,
+             const boid_params* bp, void* stream, float* density, void* accel, uint32_t* ncount, uint32_t* touched) {
+  if (!ctx) return SPH_E_INVALID;
+  if (n > ctx->p.max_particles) return fail(ctx, SPH_E_INVALID, "n exceeds max_particles");
+  if (n_boid > ctx->p.max_boids) return fail(ctx, SPH_E_INVALID, "n_boid exceeds max_boids");
+  if (n > 0 && (!pos || !vel || !aligned16(pos) || !aligned16(vel) || !aligned16(accel)))
+    return fail(ctx, SPH_E_INVALID, "pos/vel/accel must be 16-byte aligned device pointers");
+  if (n_boid > 0 && (!bpos || !bvel || !bp || !aligned16(bpos) || !aligned16(bvel)))
+    return fail(ctx, SPH_E_INVALID, "boid arrays / params missing or misaligned");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  if (!(ctx->grid_fresh && ctx->grid_pos == pos && ctx->grid_vel == vel && ctx->grid_n == n))
+    build_grid(ctx, pos, vel, n, s);
+  ctx->boid_state = false;
+  if (n_boid > 0) {
+    int rc = set_boid_params(ctx, bp);
+    if (rc != SPH_OK) return rc;
+    launch_build_grid(ctx->bc.grid, ctx->bg, (const float4*)bpos, (const float4*)bvel, n_boid, ctx->scan, s,
+                      &ctx->launches);  // S7 / K14: Boid Space hash, same machinery as the particle grid
+  }
+  launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, s, &ctx->launches);
+  if (n_boid > 0) launch_boid_density(ctx->sc, ctx->pg, ctx->bg, n_boid, ctx->rho_bS, s, &ctx->launches);
+  launch_force_integrate(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS,
+                         ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, s, &ctx->launches);
+  ctx->grid_fresh = false;  // positions moved
+  ctx->step_state = true;   // pg / rhoS still describe the step-start state (for boid_step)
+  if (n_boid > 0) {
+    ctx->boid_state = true;
+    ctx->boid_pos = bpos;
+    ctx->boid_n = n_boid;
+  }
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+int boid_step(sph_ctx* ctx, const boid_params* bp, void* bpos, void* bvel, uint32_t n_boid, void* stream,
+              void* dv_parts) {
+  if (!ctx) return SPH_E_INVALID;
+  if (n_boid == 0) return SPH_OK;
+  if (!bp || !bpos || !bvel || !aligned16(bpos) || !aligned16(bvel) || !aligned16(dv_parts))
+    return fail(ctx, SPH_E_INVALID, "boid arrays / params missing or misaligned");
+  if (!(ctx->step_state && ctx->boid_state && ctx->boid_pos == bpos && ctx->boid_n == n_boid))
+    return fail(ctx, SPH_E_STALE_GRID, "boid_step must follow sph_step called with the same boids");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  const GridDesc keep = ctx->bc.grid;
+  int rc = set_boid_params(ctx, bp);  // weights may differ from sph_step's; the grid must not
+  if (rc != SPH_OK) return rc;
+  if (memcmp(&keep, &ctx->bc.grid, sizeof(GridDesc)) != 0)
+    return fail(ctx, SPH_E_STALE_GRID, "boid ranges / space changed since sph_step");
+  launch_boid_step(ctx->sc, ctx->bc, ctx->pg, ctx->bg, ctx->grid_n, n_boid, ctx->rhoS, ctx->rho_bS, (float4*)bpos,
+                   (float4*)bvel, (float4*)dv_parts, s, &ctx->launches);
+  ctx->boid_state = false;  // boids moved
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi) {
+  if (!ctx) return SPH_E_INVALID;
+  McConst m;
+  int rc = make_mc(ctx, mp, m);
+  if (rc != SPH_OK) return rc;
+  if (!phi) return fail(ctx, SPH_E_INVALID, "phi is NULL");
+  if (!ctx->grid_fresh) return fail(ctx, SPH_E_STALE_GRID, "mc needs sph_build_grid on the current positions");
+  CK(cudaSetDevice(ctx->device));
+  launch_voxel_sdf(ctx->sc, m, ctx->pg, phi, (cudaStream_t)stream, &ctx->launches);
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+int mc_polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, void* stream, float* tris,
+                  uint32_t tri_capacity, uint32_t* n_tris_host, uint32_t* n_tris_dev) {
+  if (!ctx) return SPH_E_INVALID;
+  McConst m;
+  int rc = make_mc(ctx, mp, m);
+  if (rc != SPH_OK) return rc;
+  if (!phi || (tri_capacity > 0 && !tris)) return fail(ctx, SPH_E_INVALID, "phi / tris is NULL");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  launch_mc_polygonise(m, phi, tris, tri_capacity, ctx->n_tris_dev, ctx->scan, s, &ctx->launches);
+  if (n_tris_dev) CK(cudaMemcpyAsync(n_tris_dev, ctx->n_tris_dev, 4, cudaMemcpyDeviceToDevice, s));
+  CK(cudaGetLastError());
+  if (n_tris_host) {
+    CK(cudaMemcpyAsync(n_tris_host, ctx->n_tris_dev, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    if (*n_tris_host > tri_capacity) return fail(ctx, SPH_E_CAPACITY, "triangle buffer too small");
+  }
+  return SPH_OK;
+}
+
+int mc_extract(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi, float* tris, uint32_t tri_capacity,
+               uint32_t* n_tris_host) {
+  if (!ctx) return SPH_E_INVALID;
+  float* field = phi ? phi : ctx->phi;
+  int rc = mc_voxel_sdf(ctx, mp, stream, field);
+  if (rc != SPH_OK) return rc;
+  return mc_polygonise(ctx, mp, field, stream, tris, tri_capacity, n_tris_host, nullptr);
+}
+
+int sph_simulate_host(sph_ctx* ctx, float* pos_host, float* vel_host, uint32_t n, float* bpos_host, float* bvel_host,
+                      uint32_t n_boid, const boid_params* bp, uint32_t steps, const mc_params* mp, float* tris_host,
+                      uint32_t tri_capacity, uint32_t* n_tris_host) {
+  if (!ctx) return SPH_E_INVALID;
+  if (n > ctx->p.max_particles || n_boid > ctx->p.max_boids) return fail(ctx, SPH_E_INVALID, "n exceeds capacity");
+  if (n > 0 && (!pos_host || !vel_host)) return fail(ctx, SPH_E_INVALID, "host state is NULL");
+  if (n_boid > 0 && (!bpos_host || !bvel_host || !bp)) return fail(ctx, SPH_E_INVALID, "host boid state is NULL");
+  CK(cudaSetDevice(ctx->device));
+  if (!ctx->h_pos) {
+    const size_t nn = std::max<uint32_t>(ctx->p.max_particles, 1), nb = std::max<uint32_t>(ctx->p.max_boids, 1);
+    CK(cudaMalloc(&ctx->h_pos, nn * 16));
+    CK(cudaMalloc(&ctx->h_vel, nn * 16));
+    CK(cudaMalloc(&ctx->h_bpos, nb * 16));
+    CK(cudaMalloc(&ctx->h_bvel, nb * 16));
+  }
+  if (mp && tri_capacity > ctx->h_tris_cap) {
+    cudaFree(ctx->h_tris);
+    ctx->h_tris = nullptr;
+    CK(cudaMalloc(&ctx->h_tris, (size_t)tri_capacity * 36));
+    ctx->h_tris_cap = tri_capacity;
+  }
+  cudaStream_t s = nullptr;
+  CK(cudaMemcpyAsync(ctx->h_pos, pos_host, (size_t)n * 16, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->h_vel, vel_host, (size_t)n * 16, cudaMemcpyHostToDevice, s));
+  if (n_boid) {
+    CK(cudaMemcpyAsync(ctx->h_bpos, bpos_host, (size_t)n_boid * 16, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(ctx->h_bvel, bvel_host, (size_t)n_boid * 16, cudaMemcpyHostToDevice, s));
+  }
+  for (uint32_t t = 0; t < steps; ++t) {
+    int rc = sph_build_grid(ctx, ctx->h_pos, ctx->h_vel, n, s, nullptr, nullptr, nullptr);
+    if (rc != SPH_OK) return rc;
+    rc = sph_step(ctx, ctx->h_pos, ctx->h_vel, n, ctx->h_bpos, ctx->h_bvel, n_boid, bp, s, nullptr, nullptr, nullptr,
+                  nullptr);
+    if (rc != SPH_OK) return rc;
+    rc = boid_step(ctx, bp, ctx->h_bpos, ctx->h_bvel, n_boid, s, nullptr);
+    if (rc != SPH_OK) return rc;
+  }
+  int result = SPH_OK;
+  uint32_t nt = 0;
+  if (mp) {
+    int rc = sph_build_grid(ctx, ctx->h_pos, nullptr, n, s, nullptr, nullptr, nullptr);
+    if (rc != SPH_OK) return rc;
+    rc = mc_extract(ctx, mp, s, nullptr, ctx->h_tris, tri_capacity, &nt);
+    if (rc != SPH_OK && rc != SPH_E_CAPACITY) return rc;
+    result = rc;
+    const uint32_t got = std::min(nt, tri_capacity);
+    if (got && tris_host) CK(cudaMemcpyAsync(tris_host, ctx->h_tris, (size_t)got * 36, cudaMemcpyDeviceToHost, s));
+  }
+  if (n_tris_host) *n_tris_host = nt;
+  CK(cudaMemcpyAsync(pos_host, ctx->h_pos, (size_t)n * 16, cudaMemcpyDeviceToHost, s));
+  CK(cudaMemcpyAsync(vel_host, ctx->h_vel, (size_t)n * 16, cudaMemcpyDeviceToHost, s));
+  if (n_boid) {
+    CK(cudaMemcpyAsync(bpos_host, ctx->h_bpos, (size_t)n_boid * 16, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(bvel_host, ctx->h_bvel, (size_t)n_boid * 16, cudaMemcpyDeviceToHost, s));
+  }
+  CK(cudaStreamSynchronize(s));
+  return result;
+}
+
+}  // extern "C"

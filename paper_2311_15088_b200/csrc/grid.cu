@@ -1,0 +1,137 @@
+// grid.cu -- S1-S5: cell hash, histogram, device-wide exclusive scan, counting-sort scatter, reorder.
+// P:389-395 (get_cell, hash), P:421-439 + P:467 (Listing 8: set_particle_count, count_sort_particle_index).
+#include "kernels.h"
+
+namespace sphb {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kScanItems = 8;                     // cells per thread in the scan
+constexpr int kScanTile = kThreads * kScanItems;  // 2048 cells per tile
+
+// S1 + S2 (P:426-432 set_particle_count): key = hash(get_cell(p)); rank = atomicAdd(count[key], 1).
+__global__ void __launch_bounds__(kThreads) k_hash_count(GridDesc g, const float4* __restrict__ pos, uint32_t n,
+                                                         uint32_t* __restrict__ key, uint32_t* __restrict__ rank,
+                                                         uint32_t* __restrict__ count) {
+  const uint32_t i = blockIdx.x * kThreads + threadIdx.x;
+  if (i >= n) return;
+  const float4 p = __ldg(pos + i);
+  const int cx = cell_coord(p.x, g.lo[0], g.cell, g.dim[0]);
+  const int cy = cell_coord(p.y, g.lo[1], g.cell, g.dim[1]);
+  const int cz = cell_coord(p.z, g.lo[2], g.cell, g.dim[2]);
+  const uint32_t k = cell_hash(g, cx, cy, cz);
+  key[i] = k;
+  rank[i] = atomicAdd(count + k, 1u);
+}
+
+// S3 (D:A-OFFSET): exclusive scan of the histogram in ONE pass -- block-local scan plus
+// decoupled look-back over tile aggregates -- instead of the paper's up-sweep / down-sweep.  Scans C+1
+// entries (entry C counts 0) so that start[C] = total, and clears the histogram for the next build.
+__global__ void __launch_bounds__(kThreads) k_scan_cells(uint32_t* __restrict__ count, uint32_t* __restrict__ start,
+                                                         uint32_t C, ScanState st) {
+  __shared__ uint32_t s_scan[33];
+  __shared__ uint32_t s_tile, s_base;
+  if (threadIdx.x == 0) s_tile = atomicAdd(st.ticket, 1u) - st.ticket_base;
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const uint32_t first = tile * kScanTile + threadIdx.x * kScanItems;
+  const bool full = first + kScanItems <= C;
+  uint32_t v[kScanItems];
+  if (full) {  // two 16-byte loads, two 16-byte clears
+    const uint4 a = *reinterpret_cast<const uint4*>(count + first);
+    const uint4 b = *reinterpret_cast<const uint4*>(count + first + 4);
+    v[0] = a.x, v[1] = a.y, v[2] = a.z, v[3] = a.w, v[4] = b.x, v[5] = b.y, v[6] = b.z, v[7] = b.w;
+    *reinterpret_cast<uint4*>(count + first) = make_uint4(0, 0, 0, 0);
+    *reinterpret_cast<uint4*>(count + first + 4) = make_uint4(0, 0, 0, 0);
+  } else {
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+      v[k] = 0u;
+      if (first + k < C) {
+        v[k] = count[first + k];
+        count[first + k] = 0u;
+      }
+    }
+  }
+  uint32_t sum = 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) sum += v[k];
+  uint32_t total;
+  uint32_t excl = block_exclusive_scan(sum, s_scan, &total);
+  if (threadIdx.x < 32) {
+    const uint32_t base = lookback_exclusive(st, tile, total);
+    if (threadIdx.x == 0) s_base = base;
+  }
+  __syncthreads();
+  excl += s_base;
+  uint32_t o[kScanItems];
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    o[k] = excl;
+    excl += v[k];
+  }
+  if (full) {
+    *reinterpret_cast<uint4*>(start + first) = make_uint4(o[0], o[1], o[2], o[3]);
+    *reinterpret_cast<uint4*>(start + first + 4) = make_uint4(o[4], o[5], o[6], o[7]);
+  } else {
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k)
+      if (first + k <= C) start[first + k] = o[k];
+  }
+}
+
+// S4a (P:433-439 count_sort_particle_index): slot_id[start[key] + rank] = id.
+__global__ void __launch_bounds__(kThreads) k_scatter(const uint32_t* __restrict__ key, const uint32_t* __restrict__ rank,
+                                                      const uint32_t* __restrict__ start, uint32_t n,
+                                                      uint32_t* __restrict__ slot_id) {
+  const uint32_t i = blockIdx.x * kThreads + threadIdx.x;
+  if (i >= n) return;
+  slot_id[__ldg(start + __ldg(key + i)) + __ldg(rank + i)] = i;
+}
+
+// S4b: the atomic ranks are in arrival order; the canonical order is ascending id inside a cell
+// (D:A-SORT).  Each slot counts the smaller ids of its cell's run (a run is ~8 ids) and moves there, carrying
+// the physical copies of pos / vel (the paper keeps an index indirection instead).
+__global__ void __launch_bounds__(kThreads) k_reorder(const uint32_t* __restrict__ key, const uint32_t* __restrict__ start,
+                                                      const uint32_t* __restrict__ slot_id,
+                                                      const float4* __restrict__ pos, const float4* __restrict__ vel,
+                                                      uint32_t n, uint32_t* __restrict__ perm,
+                                                      float4* __restrict__ posS, float4* __restrict__ velS) {
+  const uint32_t s = blockIdx.x * kThreads + threadIdx.x;
+  if (s >= n) return;
+  const uint32_t id = __ldg(slot_id + s);
+  const uint32_t c = __ldg(key + id);
+  const uint32_t s0 = __ldg(start + c), s1 = __ldg(start + c + 1);
+  uint32_t smaller = 0;
+  for (uint32_t t = s0; t < s1; ++t) smaller += (__ldg(slot_id + t) < id) ? 1u : 0u;
+  const uint32_t dst = s0 + smaller;
+  perm[dst] = id;
+  posS[dst] = __ldg(pos + id);
+  if (vel) velS[dst] = __ldg(vel + id);
+}
+
+}  // namespace
+
+uint32_t grid_scan_tiles(uint32_t C) { return (C + 1 + kScanTile - 1) / kScanTile; }
+
+void launch_build_grid(const GridDesc& g, const GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
+                       ScanState& scan, cudaStream_t s, uint64_t* launches) {
+  const uint32_t blocks = (n + kThreads - 1) / kThreads;
+  if (n > 0) {
+    k_hash_count<<<blocks, kThreads, 0, s>>>(g, pos, n, b.key, b.rank, b.count);
+    ++*launches;
+  }
+  const uint32_t tiles = grid_scan_tiles(g.C);
+  scan.epoch += 1;
+  k_scan_cells<<<tiles, kThreads, 0, s>>>(b.count, b.start, g.C, scan);
+  scan.ticket_base += tiles;
+  ++*launches;
+  if (n > 0) {
+    k_scatter<<<blocks, kThreads, 0, s>>>(b.key, b.rank, b.start, n, b.slot_id);
+    k_reorder<<<blocks, kThreads, 0, s>>>(b.key, b.start, b.slot_id, pos, vel, n, b.perm, b.posS, b.velS);
+    *launches += 2;
+  }
+}
+
+}  // namespace sphb

@@ -1,0 +1,74 @@
+// kernels.h -- host-side launchers of libsphboid's CUDA kernels (internal; the public ABI is include/sphboid.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "common.cuh"
+
+namespace sphb {
+
+struct SphConst {       // values every SPH kernel needs, precomputed once on the host
+  GridDesc grid;        // particle grid, cell = h
+  float h, h2;          // h2 = h*h in binary32 (D:A-FP)
+  float mass, rho0, stiffness, viscosity;
+  float mass_c6;        // m * 315/(64 pi h^9), binary64 rounded once
+  float gravity[3], dt, damp;
+  float box_min[3], box_max[3];
+};
+
+struct BoidConst {
+  GridDesc grid;        // Boid Space grid, cell = max(visible, protect, push radius) (D:C-BGRID)
+  float protect, visible, prot2, vis2;
+  float w_sep, w_ali, w_coh, min_speed, max_speed, edge_turn, sph_factor;
+  float push_radius, w_push;
+  float space_min[3], space_max[3];
+  int reach_push;       // ceil(push_radius / h) particle cells
+};
+
+struct McConst {
+  float origin[3], spacing;
+  uint32_t G;
+  float R, R2, rbar, iso;
+  int reach;            // ceil(R / h) particle cells (D:A-R)
+};
+
+// Scratch of one grid (particles or boids).
+struct GridBuf {
+  uint32_t* key;        // [n] cell of each point (caller order)
+  uint32_t* rank;       // [n] arrival rank inside the cell (atomic order)
+  uint32_t* count;      // [C] histogram, zero between builds
+  uint32_t* start;      // [C+1] exclusive starts
+  uint32_t* slot_id;    // [n] ids in arrival order
+  uint32_t* perm;       // [n] sorted slot -> id, ascending id inside a cell (D:A-SORT)
+  float4* posS;         // [n] cell-sorted copies
+  float4* velS;
+};
+
+// grid.cu
+void launch_build_grid(const GridDesc& g, const GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
+                       ScanState& scan, cudaStream_t s, uint64_t* launches);
+uint32_t grid_scan_tiles(uint32_t C);
+// sph.cu
+void launch_density(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
+                    uint32_t* ncount_out, cudaStream_t s, uint64_t* launches);
+void launch_boid_density(const SphConst& c, const GridBuf& pg, const GridBuf& bg, uint32_t nb, float* rho_bS,
+                         cudaStream_t s, uint64_t* launches);
+void launch_force_integrate(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg,
+                            uint32_t n, uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos,
+                            float4* vel, float4* accel_out, uint32_t* touched_out, cudaStream_t s,
+                            uint64_t* launches);
+// boid.cu
+void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
+                      uint32_t nb, const float* rhoS, const float* rho_bS, float4* bpos, float4* bvel,
+                      float4* dv_parts, cudaStream_t s, uint64_t* launches);
+// mc.cu
+void upload_mc_tables();
+void mc_table_host(int8_t* tri, uint8_t* ntri);
+void launch_voxel_sdf(const SphConst& c, const McConst& m, const GridBuf& pg, float* phi, cudaStream_t s,
+                      uint64_t* launches);
+void launch_mc_polygonise(const McConst& m, const float* phi, float* tris, uint32_t capacity, uint32_t* n_tris_dev,
+                          ScanState& scan, cudaStream_t s, uint64_t* launches);
+uint32_t mc_num_tiles(uint32_t G);
+
+}  // namespace sphb

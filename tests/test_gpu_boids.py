@@ -1,0 +1,94 @@
+"""Parity of S7, S11-S13 (boid grid, probe density, boid rules, fluid->boid force, move) against the oracle."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import refbind as R
+from paper_2311_15088_b200 import binding as B
+from paper_2311_15088_b200 import workloads as W
+from tests.gpuutil import Sim, dev, vec_err
+
+pytestmark = pytest.mark.gpu
+
+
+def _frame(cfg, pos, vel, bpos, bvel):
+    ref = R.step(cfg["sph"], pos, vel, bpos, bvel, cfg["boid"])
+    refb = R.boid_step(cfg["sph"], cfg["boid"], pos, vel, ref["density"], bpos, bvel)
+    with Sim(cfg) as sim:
+        dbp, dbv = dev(bpos), dev(bvel)
+        sim.step(dev(pos), dev(vel), dbp, dbv, cfg["boid"])
+        out = sim.boid_step(cfg["boid"], dbp, dbv)
+    return refb, out
+
+
+def _compare(refb, out):
+    bad, worst = vec_err(out["bvel"][:, :3], refb["bvel"][:, :3])
+    assert bad == 0, ("bvel", bad, worst)
+    bad, worst = vec_err(out["bpos"][:, :3], refb["bpos"][:, :3])
+    assert bad == 0, ("bpos", bad, worst)
+    scale = np.abs(refb["dv_parts"]).max() + 1e-30
+    assert np.abs(out["dv_parts"] - refb["dv_parts"]).max() <= 1e-5 * scale + 1e-9
+
+
+@pytest.mark.parametrize("idx,scale", [(1, None), (2, None), (3, 2), (4, 4), (5, 4)])
+def test_boid_step_matches_oracle(idx, scale):
+    cfg = W.config(idx, scale=scale)
+    vel0 = W.uniform_box(cfg["n"], (-0.2,) * 3, (0.2,) * 3, 1, 30)
+    refb, out = _frame(cfg, cfg["pos"], vel0, cfg["bpos"], cfg["bvel"])
+    _compare(refb, out)
+    if idx in (3, 4, 5):
+        assert np.abs(refb["dv_parts"][:, 3]).max() > 0  # fluid -> boid force is live
+
+
+def test_boids_outside_space_fast_and_slow():
+    cfg = W.config(1)
+    bp = dict(cfg["boid"], min_speed=0.05)
+    cfg = dict(cfg, boid=bp)
+    bpos = W.uniform_box(200, (-0.2, -0.2, -0.2), (1.2, 1.2, 1.2), 3, 10)  # some outside the Boid Space: edge rule
+    bvel = W.uniform_box(200, (-1.0,) * 3, (1.0,) * 3, 3, 20)              # many above max_speed
+    bvel[:20, :3] *= 0.01                                                  # some below min_speed
+    bvel[20] = 0.0
+    cfg["n_boid"] = 200
+    refb, out = _frame(cfg, cfg["pos"], cfg["vel"], bpos, bvel)
+    _compare(refb, out)
+
+
+def test_single_boid_and_clustered_boids():
+    cfg = W.config(3, scale=4)
+    one_p, one_v = cfg["bpos"][:1].copy(), cfg["bvel"][:1].copy()
+    refb, out = _frame(dict(cfg, n_boid=1), cfg["pos"], cfg["vel"], one_p, one_v)
+    _compare(refb, out)
+    h = cfg["sph"]["h"]
+    bpos = W.uniform_ball(900, (0.12, 0.12, 0.12), 2.0 * h, 5, 10)  # hundreds of boid neighbours each
+    bvel = W.uniform_box(900, (-0.1,) * 3, (0.1,) * 3, 5, 20)
+    refb, out = _frame(dict(cfg, n_boid=900), cfg["pos"], cfg["vel"], bpos, bvel)
+    _compare(refb, out)
+
+
+def test_boid_step_requires_matching_sph_step():
+    cfg = W.config(1)
+    with Sim(cfg) as sim:
+        bpos, bvel = dev(cfg["bpos"]), dev(cfg["bvel"])
+        with pytest.raises(B.SphError) as e:
+            B.boid_step(sim.ctx, cfg["boid"], bpos, bvel)
+        assert e.value.code == B.SPH_E_STALE_GRID
+        sim.step(dev(cfg["pos"]), dev(cfg["vel"]), bpos, bvel, cfg["boid"])
+        B.boid_step(sim.ctx, cfg["boid"], bpos, bvel)
+        with pytest.raises(B.SphError):  # the boids moved: a second boid_step in the same frame is stale
+            B.boid_step(sim.ctx, cfg["boid"], bpos, bvel)
+        torch.cuda.synchronize()
+
+
+def test_two_frames_free_running():
+    cfg = W.config(3, scale=4)
+    pos, vel, bpos, bvel = cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"]
+    with Sim(cfg) as sim:
+        dp, dv, dbp, dbv = dev(pos), dev(vel), dev(bpos), dev(bvel)
+        for _ in range(2):
+            ref = R.step(cfg["sph"], pos, vel, bpos, bvel, cfg["boid"])
+            refb = R.boid_step(cfg["sph"], cfg["boid"], pos, vel, ref["density"], bpos, bvel)
+            pos, vel, bpos, bvel = ref["pos"], ref["vel"], refb["bpos"], refb["bvel"]
+            sim.step(dp, dv, dbp, dbv, cfg["boid"])
+            out = sim.boid_step(cfg["boid"], dbp, dbv)
+        bad, worst = vec_err(out["bvel"][:, :3], bvel[:, :3], rel=2e-5, abs_=2e-6)
+        assert bad == 0, (bad, worst)

@@ -1,0 +1,131 @@
+"""Parity of S14-S17 (voxel SDF, marching cubes) against the oracle.
+
+Stage-isolated (oracle phi fed to the CUDA polygoniser): triangle count, order and vertices bit-exact.
+phi itself: |d| <= 1e-5 h.  End to end: counts may differ only at cubes that touch a corner whose
+|phi - iso| is below the phi tolerance; those are counted and must be few.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import refbind as R
+from paper_2311_15088_b200 import binding as B
+from paper_2311_15088_b200 import workloads as W
+from tests.gpuutil import Sim, dev
+
+pytestmark = pytest.mark.gpu
+
+
+def _polygonise_gpu(sim, mp, phi_np, capacity):
+    tris = torch.zeros(max(capacity, 1), 3, 3, device="cuda")
+    nt = B.mc_polygonise(sim.ctx, mp, dev(phi_np), tris)
+    return tris.cpu().numpy()[:min(nt, capacity)], nt
+
+
+@pytest.mark.parametrize("idx,scale", [(1, None), (2, None), (3, 2), (4, 4)])
+def test_sdf_and_polygonise_on_configs(idx, scale):
+    cfg = W.config(idx, scale=scale)
+    mp = W.mc_params(cfg)
+    G, h = mp["n_point_per_axis"], cfg["sph"]["h"]
+    phi_ref = R.voxel_sdf(cfg["sph"], mp, cfg["pos"])
+    tris_ref, nt_ref, _ = R.mc_polygonise(mp, phi_ref)
+    with Sim(cfg, G=G) as sim:
+        B.sph_build_grid(sim.ctx, dev(cfg["pos"]))
+        phi = torch.zeros(G ** 3, device="cuda")
+        B.mc_voxel_sdf(sim.ctx, mp, phi)
+        phi_gpu = phi.cpu().numpy()
+        assert np.abs(phi_gpu - phi_ref).max() <= 1e-5 * h
+        # stage-isolated: bit-exact
+        tris, nt = _polygonise_gpu(sim, mp, phi_ref, nt_ref + 7)
+        assert nt == nt_ref and nt > 0
+        assert np.array_equal(tris, tris_ref)
+        # end to end through mc_extract (library scratch phi)
+        buf = torch.zeros(nt_ref + 1000, 3, 3, device="cuda")
+        nt2 = B.mc_extract(sim.ctx, mp, buf)
+        risky = np.abs(phi_ref - mp["iso"]) <= 1e-5 * h
+        assert abs(nt2 - nt_ref) <= 5 * 8 * int(risky.sum())
+        if not risky.any():
+            assert nt2 == nt_ref and np.abs(buf.cpu().numpy()[:nt2] - tris_ref).max() <= 1e-5 * mp["spacing"]
+
+
+def test_polygonise_random_noise_all_cases_ragged_tiles():
+    # white noise: all 256 cases; G-1 = 22 -> 10648 cubes = 10 tiles + a ragged tail
+    G = 23
+    rng = np.random.default_rng(5)
+    phi = rng.standard_normal(G ** 3).astype(np.float32)
+    mp = dict(origin=(0.1, -0.2, 0.3), spacing=0.013, n_point_per_axis=G, radius=0.05, particle_radius=0.02, iso=0.1)
+    tris_ref, nt_ref, cases = R.mc_polygonise(mp, phi, want_cases=True)
+    assert len(np.unique(cases)) == 256
+    cfg = dict(sph=W.config(1)["sph"], n=1)
+    with Sim(cfg, G=G) as sim:
+        tris, nt = _polygonise_gpu(sim, mp, phi, nt_ref)
+        assert nt == nt_ref and np.array_equal(tris, tris_ref)
+        # capacity smaller than needed: required count still reported, nothing past capacity written
+        cap = nt_ref // 3
+        buf = torch.full((cap + 50, 3, 3), -7.0, device="cuda")
+        m = B._fill(B.McParams, mp)
+        import ctypes as C
+        got = C.c_uint32(0)
+        rc = B.lib().mc_polygonise(sim.ctx, C.byref(m), C.c_void_p(dev(phi).data_ptr()), None,
+                                   C.c_void_p(buf.data_ptr()), cap, C.byref(got), None)
+        assert rc == B.SPH_E_CAPACITY and got.value == nt_ref
+        out = buf.cpu().numpy()
+        assert np.array_equal(out[:cap], tris_ref[:cap]) and np.all(out[cap:] == -7.0)
+
+
+@pytest.mark.parametrize("G", [2, 3, 17])
+def test_polygonise_tiny_and_empty_grids(G):
+    mp = dict(origin=(0.0, 0.0, 0.0), spacing=0.1, n_point_per_axis=G, radius=0.05, particle_radius=0.02, iso=0.0)
+    cfg = dict(sph=W.config(1)["sph"], n=1)
+    with Sim(cfg, G=G) as sim:
+        phi = np.ones(G ** 3, np.float32)  # nothing below iso: zero triangles
+        _, nt = _polygonise_gpu(sim, mp, phi, 4)
+        assert nt == 0
+        phi[0] = -1.0  # one corner below: exactly one triangle
+        tris, nt = _polygonise_gpu(sim, mp, phi, 4)
+        ref, nt_ref, _ = R.mc_polygonise(mp, phi)
+        assert nt == nt_ref == 1 and np.array_equal(tris, ref)
+
+
+def test_sdf_requires_fresh_grid_and_empty_space():
+    cfg = W.config(1)
+    mp = W.mc_params(cfg)
+    G = mp["n_point_per_axis"]
+    with Sim(cfg, G=G) as sim:
+        phi = torch.zeros(G ** 3, device="cuda")
+        with pytest.raises(B.SphError) as e:
+            B.mc_voxel_sdf(sim.ctx, mp, phi)
+        assert e.value.code == B.SPH_E_STALE_GRID
+        pos, vel = dev(cfg["pos"]), dev(cfg["vel"])
+        sim.step(pos, vel)
+        with pytest.raises(B.SphError):  # positions moved since the grid was built
+            B.mc_voxel_sdf(sim.ctx, mp, phi)
+        B.sph_build_grid(sim.ctx, pos)
+        B.mc_voxel_sdf(sim.ctx, mp, phi)
+        far = phi.view(G, G, G)[G - 1, G - 1, G - 1].item()  # corner (1,1,1): no particle within R
+        assert far == np.float32(mp["radius"]) - np.float32(mp["particle_radius"])
+
+
+def test_full_size_mc_config4_sampled():
+    # BASELINE.json's headline surface pass (1 048 576 particles, 256^3 corners): phi on sampled z-planes against the
+    # oracle, and properties that hold at any size for the mesh (count = sum ntri[case], closed away from the grid border)
+    cfg = W.config(4)
+    mp = W.mc_params(cfg)
+    G, h = mp["n_point_per_axis"], cfg["sph"]["h"]
+    with Sim(cfg, G=G) as sim:
+        B.sph_build_grid(sim.ctx, dev(cfg["pos"]))
+        phi = torch.zeros(G ** 3, device="cuda")
+        B.mc_voxel_sdf(sim.ctx, mp, phi)
+        phi_gpu = phi.cpu().numpy().reshape(G, G, G)
+        for k in (0, 37, 100, 127, 128, 200, 255):
+            plane = dict(mp, origin=(mp["origin"][0], mp["origin"][1],
+                                     float(np.float32(mp["origin"][2]) + np.float32(k) * np.float32(mp["spacing"]))))
+            ref = R.voxel_sdf(cfg["sph"], dict(plane, n_point_per_axis=G), cfg["pos"]) if False else None
+        # whole-field comparison is affordable on the oracle (16.7M corners): do it outright
+        phi_ref = R.voxel_sdf(cfg["sph"], mp, cfg["pos"]).reshape(G, G, G)
+        assert np.abs(phi_gpu - phi_ref).max() <= 1e-5 * h
+        tris_ref, nt_ref, _ = R.mc_polygonise(mp, phi_gpu.reshape(-1))
+        buf = torch.zeros(nt_ref + 10, 3, 3, device="cuda")
+        nt = B.mc_polygonise(sim.ctx, mp, phi, buf)
+        assert nt == nt_ref
+        assert np.array_equal(buf.cpu().numpy()[:nt], tris_ref)

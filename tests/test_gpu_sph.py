@@ -1,0 +1,121 @@
+"""Parity of S6-S10 (density, neighbour count, forces, boid push, integration) against the oracle.
+
+Integers (ncount, touched) bit-exact.  Floats per particle, vector norm:
+  rho, v, x : |d| <= 1e-5 |ref| + 1e-6            a : |d| <= 1e-5 |a_ref| + 1e-6
+  step displacement x' - x : |d| <= 1e-5 |ref| + 2 ulp(box extent)   (x itself is stored in binary32)
+"""
+import numpy as np
+import pytest
+
+from oracle import refbind as R
+from paper_2311_15088_b200 import workloads as W
+from tests.gpuutil import Sim, dev, vec_err
+
+pytestmark = pytest.mark.gpu
+
+
+def _compare_step(cfg, out, ref, pos0):
+    assert np.array_equal(out["ncount"], ref["ncount"])
+    assert np.array_equal(out["touched"], ref["touched"])
+    bad, worst = vec_err(out["density"], ref["density"])
+    assert bad == 0, ("density", bad, worst)
+    bad, worst = vec_err(out["accel"][:, :3], ref["accel"][:, :3])
+    assert bad == 0, ("accel", bad, worst)
+    bad, worst = vec_err(out["vel"][:, :3], ref["vel"][:, :3])
+    assert bad == 0, ("vel", bad, worst)
+    bad, worst = vec_err(out["pos"][:, :3], ref["pos"][:, :3])
+    assert bad == 0, ("pos", bad, worst)
+    ulp = 2.0 * np.spacing(np.float32(max(cfg["sph"]["box_max"])))
+    bad, worst = vec_err(out["pos"][:, :3] - pos0[:, :3], ref["pos"][:, :3] - pos0[:, :3], abs_=float(ulp) * np.sqrt(3))
+    assert bad == 0, ("displacement", bad, worst)
+    # the 4th lanes are carried through
+    assert np.array_equal(out["pos"][:, 3], pos0[:, 3])
+
+
+@pytest.mark.parametrize("idx,scale", [(1, None), (2, None), (3, 2), (4, 4), (5, 4)])
+def test_single_step_matches_oracle(idx, scale):
+    cfg = W.config(idx, scale=scale)
+    vel0 = W.uniform_box(cfg["n"], (-0.2,) * 3, (0.2,) * 3, 1, 30)
+    pos0 = cfg["pos"].copy()
+    pos0[:, 3] = np.arange(cfg["n"], dtype=np.float32)  # payload lane must survive
+    ref = R.step(cfg["sph"], pos0, vel0, cfg["bpos"], cfg["bvel"], cfg["boid"])
+    with Sim(cfg) as sim:
+        out = sim.step(dev(pos0), dev(vel0), dev(cfg["bpos"]), dev(cfg["bvel"]), cfg["boid"])
+    _compare_step(cfg, out, ref, pos0)
+    if idx in (3, 4, 5):
+        assert ref["touched"].max() > 0  # the coupling path really ran
+
+
+def test_step_without_boids_and_explicit_grid():
+    cfg = W.config(1)
+    ref = R.step(cfg["sph"], cfg["pos"], cfg["vel"])
+    with Sim(cfg) as sim:
+        pos, vel = dev(cfg["pos"]), dev(cfg["vel"])
+        sim.build_grid(pos, vel)  # sph_step must reuse this grid (same pointers), result identical either way
+        out = sim.step(pos, vel)
+    _compare_step(cfg, out, ref, cfg["pos"])
+    assert not out["touched"].any()
+
+
+def test_teacher_forced_ten_steps_config1():
+    # D:A-MULTI (i): feed the oracle's state to the GPU at every step, single-step tolerances each time
+    cfg = W.config(1)
+    pos, vel = cfg["pos"], cfg["vel"]
+    with Sim(cfg) as sim:
+        for _ in range(10):
+            ref = R.step(cfg["sph"], pos, vel, cfg["bpos"], cfg["bvel"], cfg["boid"])
+            out = sim.step(dev(pos), dev(vel), dev(cfg["bpos"]), dev(cfg["bvel"]), cfg["boid"])
+            _compare_step(cfg, out, ref, pos)
+            pos, vel = ref["pos"], ref["vel"]
+
+
+def test_free_running_ten_steps_config1_bounded_divergence():
+    # D:A-MULTI (ii): free-running states stay within a stated growing bound: eps(s) = s * (1e-5 |x| + 2e-6)
+    cfg = W.config(1)
+    rp, rv = cfg["pos"], cfg["vel"]
+    with Sim(cfg) as sim:
+        gp, gv = dev(cfg["pos"]), dev(cfg["vel"])
+        for s in range(1, 11):
+            ref = R.step(cfg["sph"], rp, rv)
+            rp, rv = ref["pos"], ref["vel"]
+            out = sim.step(gp, gv)
+            bad, worst = vec_err(out["pos"][:, :3], rp[:, :3], rel=1e-5 * s, abs_=2e-6 * s)
+            assert bad <= cfg["n"] // 10000, (s, bad, worst)
+            bad, worst = vec_err(out["vel"][:, :3], rv[:, :3], rel=1e-5 * s, abs_=2e-5 * s)
+            assert bad <= cfg["n"] // 10000, (s, bad, worst)
+
+
+def test_walls_and_out_of_box_particles():
+    cfg = W.config(1, scale=2)
+    sp = cfg["sph"]
+    pos = W.random_cloud(3000, (-0.02, -0.02, -0.02), (0.3, 0.3, 0.3), seed=7)  # some start outside the box
+    vel = W.uniform_box(3000, (-30.0,) * 3, (30.0,) * 3, 8, 30)                  # many hit a wall in one step
+    ref = R.step(sp, pos, vel)
+    with Sim(dict(sph=sp, n=3000)) as sim:
+        out = sim.step(dev(pos), dev(vel))
+    assert (ref["pos"][:, :3] == 0.0).sum() > 100
+    _compare_step(dict(sph=sp), out, ref, pos)
+    assert np.array_equal(out["pos"][:, :3] == 0.0, ref["pos"][:, :3] == 0.0)
+
+
+def test_dense_cluster_many_neighbours():
+    # degenerate: hundreds of neighbours per particle (one cell holds them all), plus coincident particles
+    sp = dict(W.config(1)["sph"])
+    pos = W.random_cloud(700, (0.40, 0.40, 0.40), (0.43, 0.43, 0.43), seed=11)
+    pos[10] = pos[11]  # coincident pair: counted as neighbours, no force between them
+    vel = W.uniform_box(700, (-0.1,) * 3, (0.1,) * 3, 12, 30)
+    ref = R.step(sp, pos, vel)
+    with Sim(dict(sph=sp, n=700)) as sim:
+        out = sim.step(dev(pos), dev(vel))
+    assert ref["ncount"].min() > 300
+    _compare_step(dict(sph=sp), out, ref, pos)
+
+
+@pytest.mark.parametrize("idx", [4, 5])
+def test_full_size_step_matches_oracle(idx):
+    # BASELINE.json's full sizes in the launch configuration bench.py times (one whole step, every particle compared)
+    cfg = W.config(idx)
+    ref = R.step(cfg["sph"], cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"], cfg["boid"])
+    with Sim(cfg) as sim:
+        out = sim.step(dev(cfg["pos"]), dev(cfg["vel"]), dev(cfg["bpos"]), dev(cfg["bvel"]), cfg["boid"])
+    _compare_step(cfg, out, ref, cfg["pos"])
