@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the per-frame particle pipeline of arXiv 2311.15088 on B200 (sm_100a).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is ONE FRAME of the whole hot path on BASELINE.json's headline
+workload (config 4: 1 048 576 fluid particles, 4 096 boids, 256^3 voxel corners):
+neighbour grid -> SPH density / forces / integration -> boid update with two-way coupling -> grid on the new
+positions -> voxel signed distance -> marching cubes.  All of it runs in libsphboid's CUDA kernels through the
+C ABI; torch supplies device memory, streams and events only.  One JSON line is printed by rank 0.
+
+  value      particle-updates/s over the whole frame = N * K / t, inputs resident in HBM
+  parts      the two halves BASELINE.json's metric names: SPH+boid particle-updates/s (S1-S13) and MC voxels/s
+             (S14-S17), each with its algorithmic GB/s and fraction of the measured HBM peak
+  e2e        the same frame through sph_simulate_host with pinned HOST buffers, copies inside the timed region
+  roofline   the dominant kernel: algorithmic bytes per launch / its average CUDA-event duration
+  kernels    every kernel: launches, average us, share of the step, algorithmic GB/s
+  cpu_baseline  the CPU oracle (oracle/, test infrastructure) timed on this box's host cores on the same workload
+
+--impl reference times the oracle alone (this tier has no reference implementation to install).
+--gpus N > 1 (under torchrun): N independent replicas, no data-path collective ("replicas only").
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particle-updates/s (whole frame: grid + SPH + boids + voxel SDF + marching cubes)"
+L2_BYTES = 126e6
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured"
+        except Exception:
+            pass
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md, clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is not None:
+            self.p.terminate()
+            try:
+                self.p.wait(timeout=5)
+            except Exception:
+                self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1]))
+                smax.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(smax), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def oracle_frame(R, W, cfg, mp, state):
+    """One frame on the CPU oracle (same order as Frame.frame).  state = [pos, vel, bpos, bvel]; returns n_tris."""
+    pos, vel, bpos, bvel = state
+    ref = R.step(cfg["sph"], pos, vel, bpos, bvel, cfg["boid"])
+    refb = R.boid_step(cfg["sph"], cfg["boid"], pos, vel, ref["density"], bpos, bvel)
+    state[:] = [ref["pos"], ref["vel"], refb["bpos"], refb["bvel"]]
+    phi = R.voxel_sdf(cfg["sph"], mp, state[0])
+    _, nt, _ = R.mc_polygonise(mp, phi)
+    return nt
+
+
+def time_oracle(cfg, mp, min_seconds, max_frames):
+    from oracle import refbind as R
+    from paper_2311_15088_b200 import workloads as W
+    state = [cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"]]
+    frames, t0 = 0, time.perf_counter()
+    per = []
+    while frames < max_frames:
+        t1 = time.perf_counter()
+        oracle_frame(R, W, cfg, mp, state)
+        per.append(time.perf_counter() - t1)
+        frames += 1
+        if time.perf_counter() - t0 >= min_seconds:
+            break
+    return frames, per, R.num_threads()
+
+
+def run_reference(args, cfg_idx):
+    """--impl reference: the CPU oracle as it stands, on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2311_15088_b200 import workloads as W
+    cfg = W.config(cfg_idx)
+    mp = W.mc_params(cfg)
+    n = cfg["n"]
+    # each "step" is one full frame of the workload on the oracle; cap the run at ~3 minutes
+    budget = 170.0
+    state = [cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"]]
+    from oracle import refbind as R
+    done_w = 0
+    t_start = time.perf_counter()
+    for _ in range(args.warmup):
+        if time.perf_counter() - t_start > budget / 4:
+            break
+        oracle_frame(R, W, cfg, mp, state)
+        done_w += 1
+    per = []
+    for _ in range(args.steps):
+        t1 = time.perf_counter()
+        oracle_frame(R, W, cfg, mp, state)
+        per.append(time.perf_counter() - t1)
+        if time.perf_counter() - t_start > budget:
+            break
+    k = len(per)
+    t = sum(per)
+    value = n * k / t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "particle-updates/s", "n_gpus": args.gpus,
+        "steps": k, "warmup": done_w, "ms_per_step": 1e3 * t / k, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg["name"], "particles": n, "boids": cfg["n_boid"], "mc_points_per_axis": cfg["G"],
+                   "note": "CPU oracle (oracle/, plain C++ with OpenMP over the outer index), one frame per step"},
+        "cpu_baseline": {"value": value, "unit": "particle-updates/s", "cores": R.num_threads(), "kind": "oracle",
+                         "sample": "%d whole frames of %s (steps requested %d, time-capped)" % (k, cfg["name"],
+                                                                                              args.steps)},
+        "e2e": {"value": value, "unit": "particle-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1-5 (4 = the headline workload)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args, args.config)
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    from paper_2311_15088_b200 import binding as B
+    from paper_2311_15088_b200 import dist as D
+    from paper_2311_15088_b200 import roofline as RF
+    from paper_2311_15088_b200 import workloads as W
+    from paper_2311_15088_b200.pipeline import Frame
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    B.lib()  # fail loudly if libsphboid.so is not built
+    ranks = D.Ranks()
+    dev = ranks.local_rank
+    torch.cuda.set_device(dev)
+    cfg = W.config(args.config, seed=ranks.rank)  # replicas differ only in the jitter / boid seed
+    n, nb, K = cfg["n"], cfg["n_boid"], args.steps
+    peak, peak_kind = measured_peak()
+
+    fr = Frame(cfg, device=dev)
+    G = fr.G
+    _, C = B.sph_grid_dims(fr.ctx)
+    for _ in range(args.warmup):
+        fr.frame()
+    torch.cuda.synchronize()
+
+    # ---- timed region: K frames, state resident in HBM -------------------------------------------------
+    sampler = ClockSampler(dev)
+    sampler.start()
+    time.sleep(0.15)
+    ranks.barrier()
+    torch.cuda.synchronize()
+    B.sph_profile_enable(fr.ctx, True)
+    launches0 = B.sph_launch_count(fr.ctx)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K + 1)]
+    ev[0].record()
+    for k in range(K):
+        fr.sim()
+        ev[2 * k + 1].record()
+        fr.surface()
+        ev[2 * k + 2].record()
+    torch.cuda.synchronize()
+    ranks.barrier()
+    launches = B.sph_launch_count(fr.ctx) - launches0
+    t_total = ev[0].elapsed_time(ev[2 * K]) * 1e-3
+    t_sim = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(K)) * 1e-3
+    t_mc = sum(ev[2 * k + 1].elapsed_time(ev[2 * k + 2]) for k in range(K)) * 1e-3
+    profile = B.sph_profile_read(fr.ctx)
+    B.sph_profile_enable(fr.ctx, False)
+    clocks = sampler.stop()
+    n_tris = B.mc_extract(fr.ctx, fr.mc, fr.tris, sync=True)  # same state as the last timed frame
+    if n_tris > fr.tri_capacity:
+        raise SystemExit("triangle buffer too small: %d > %d" % (n_tris, fr.tri_capacity))
+    cb = None
+    bpar = cfg["boid"]
+    cell_b = max(bpar["visible_range"], bpar["protect_range"], bpar["push_radius"])
+    import math
+    cb = 1
+    for a in range(3):
+        cb *= max(1, math.ceil((bpar["space_max"][a] - bpar["space_min"][a]) / cell_b))
+
+    t_max, units = ranks.combine(t_total, n * K)
+    t_sim_max, t_mc_max = ranks.reduce_max([t_sim, t_mc])
+    value = units / t_max
+    world = ranks.world
+
+    rows, dominant = RF.summarise(profile, n, C, nb, cb, G, n_tris, peak)
+    # SPH half = S1-S13 (one grid build per frame); surface half = S14-S17 (mc_extract alone)
+    sim_bytes = RF.pass_bytes(RF.SIM_KERNELS, n, C, nb, cb, G, n_tris)
+    mc_bytes = RF.pass_bytes(RF.MC_KERNELS, n, C, nb, cb, G, n_tris)
+    sim_gbs = sim_bytes * K / t_sim / 1e9
+    mc_gbs = mc_bytes * K / t_mc / 1e9
+    dom = next(r for r in rows if r["kernel"] == dominant)
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get(dominant, {}).get("dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+
+    # ---- end to end through the C ABI with HOST buffers -------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        hp = [torch.from_numpy(cfg[k].copy()).pin_memory() for k in ("pos", "vel", "bpos", "bvel")]
+        htris = torch.empty(fr.tri_capacity, 3, 3).pin_memory()
+        Ke = min(K, 10)
+        for _ in range(2):
+            B.sph_simulate_host(fr.ctx, hp[0], hp[1], hp[2], hp[3], cfg["boid"], 1, fr.mc, htris)
+        torch.cuda.synchronize()
+        ranks.barrier()
+        t0 = time.perf_counter()
+        nts = []
+        for _ in range(Ke):
+            nts.append(B.sph_simulate_host(fr.ctx, hp[0], hp[1], hp[2], hp[3], cfg["boid"], 1, fr.mc, htris))
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        ranks.barrier()
+        t_e2e_max, units_e = ranks.combine(t_e2e, n * Ke)
+        h2d = 32 * n + 32 * nb
+        d2h = 32 * n + 32 * nb + 36 * (sum(nts) // len(nts)) + 4
+        e2e = {"value": units_e / t_e2e_max, "unit": "particle-updates/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": Ke, "ms_per_step": 1e3 * t_e2e_max / Ke,
+               "api": "sph_simulate_host (pinned host pos/vel/bpos/bvel in, state + triangles out, every step)",
+               "timer": "host wall clock around the synchronous calls"}
+    fr.close()
+
+    # ---- the oracle on this box's host cores, rank 0 at N = 1 only --------------------------------------
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        frames, per, cores = time_oracle(cfg, W.mc_params(cfg), 10.0, 3)
+        cpu = {"value": n * frames / sum(per), "unit": "particle-updates/s", "cores": cores, "kind": "oracle",
+               "sample": "%d whole frame(s) of %s (%d particles, %d boids, %d^3 corners), %.1f s" %
+                         (frames, cfg["name"], n, nb, G, sum(per))}
+
+    if ranks.rank == 0:
+        state_bytes = 32 * n * 2 + 16 * n + 4 * G ** 3 + 36 * n_tris + 8 * C
+        line = {
+            "metric": METRIC, "value": value, "unit": "particle-updates/s", "n_gpus": world, "steps": K,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_max / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg["name"], "particles": n, "boids": nb, "mc_points_per_axis": G,
+                       "grid_cells": C, "triangles_last_frame": n_tris, "parallelism": "replicas x%d" % world,
+                       "l2": "no explicit flush: the frame's working set (%.0f MB) exceeds the %.0f MB L2 and "
+                             "the state changes every step" % (state_bytes / 1e6, L2_BYTES / 1e6)},
+            "parts": {
+                "sph_boid": {"value": n * K * world / t_sim_max, "unit": "particle-updates/s",
+                             "ms_per_step": 1e3 * t_sim_max / K, "algorithmic_gbs": sim_gbs,
+                             "frac_of_hbm_peak": sim_gbs / peak,
+                             "rows": "S1-S13: sph_step + boid_step + the frame's one sph_build_grid"},
+                "mc": {"value": G ** 3 * K * world / t_mc_max, "unit": "voxels/s", "ms_per_step": 1e3 * t_mc_max / K,
+                       "algorithmic_gbs": mc_gbs, "frac_of_hbm_peak": mc_gbs / peak, "rows": "S14-S17: mc_extract"},
+            },
+            "roofline": {"bound": "hbm", "kernel": dominant, "achieved": dom["gbs"], "peak": peak, "unit": "GB/s",
+                         "frac": dom["frac"], "traffic": traffic, "peak_kind": "of " + peak_kind,
+                         "bytes_per_launch": dom["bytes"], "avg_us": dom["avg_us"], "share_of_step": dom["share"]},
+            "kernels": [{"kernel": r["kernel"], "launches": r["launches"], "avg_us": round(r["avg_us"], 2),
+                         "share": round(r["share"], 4), "gbs": round(r["gbs"], 1), "frac": round(r["frac"], 4)}
+                        for r in rows],
+            "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    ranks.close()
+
+
+if __name__ == "__main__":
+    main()

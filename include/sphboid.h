@@ -138,6 +138,15 @@ void sph_mc_table(int8_t* tri_host, uint8_t* ntri_host);
 /* Number of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
 uint64_t sph_launch_count(const sph_ctx* ctx);
 
+/* Per-kernel device timing (measurement only, no effect on results).  While enabled, every kernel launch of
+ * this context is bracketed by two CUDA events recorded on the launching stream.  sph_profile_enable resets the
+ * totals.  sph_profile_read synchronises on the pending events (a host sync) and returns, for kernel
+ * `kernel_id`, the number of launches and their summed duration in milliseconds (both host pointers, optional).
+ * sph_kernel_name returns the kernel's name, or NULL once kernel_id is past the last kernel. */
+int sph_profile_enable(sph_ctx* ctx, int enable);
+int sph_profile_read(sph_ctx* ctx, uint32_t kernel_id, uint64_t* launches_host, double* total_ms_host);
+const char* sph_kernel_name(uint32_t kernel_id);
+
 #ifdef __cplusplus
 }
 #endif

@@ -81,12 +81,17 @@ def lib():
         L.sph_mc_table.restype = None
         L.sph_launch_count.argtypes = [_vp]
         L.sph_launch_count.restype = C.c_uint64
+        L.sph_profile_enable.argtypes = [_vp, C.c_int]
+        L.sph_profile_read.argtypes = [_vp, _u32, _vp, _vp]
+        L.sph_kernel_name.argtypes = [_u32]
+        L.sph_kernel_name.restype = C.c_char_p
         _lib = L
     return _lib
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "mc_voxel_sdf", "mc_polygonise", "mc_extract", "sph_simulate_host", "sph_mc_table", "sph_launch_count"]
+           "mc_voxel_sdf", "mc_polygonise", "mc_extract", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "sph_profile_read", "sph_kernel_name"]
 
 
 def _ptr(t):
@@ -145,6 +150,26 @@ def sph_grid_dims(ctx):
 
 def sph_launch_count(ctx):
     return int(lib().sph_launch_count(ctx))
+
+
+def sph_profile_enable(ctx, enable=True):
+    return _check(ctx, lib().sph_profile_enable(ctx, 1 if enable else 0))
+
+
+def sph_profile_read(ctx):
+    """{kernel name: (launches, total ms)} for every kernel that launched since sph_profile_enable."""
+    out = {}
+    k = 0
+    while True:
+        name = lib().sph_kernel_name(k)
+        if name is None:
+            break
+        n, ms = C.c_uint64(0), C.c_double(0.0)
+        _check(ctx, lib().sph_profile_read(ctx, k, C.byref(n), C.byref(ms)))
+        if n.value:
+            out[name.decode()] = (int(n.value), float(ms.value))
+        k += 1
+    return out
 
 
 def sph_mc_table():

@@ -3,6 +3,7 @@
 
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -34,13 +35,46 @@ struct sph_ctx {
   bool boid_state;       // bg/rho_bS hold the boids given to the last sph_step
   const void* boid_pos;
   uint32_t boid_n;
-  uint64_t launches;
+  Prof prof;
   char err[256];
   // staging for the *_host entry point
   float4 *h_pos, *h_vel, *h_bpos, *h_bvel;
   float* h_tris;
   uint32_t h_tris_cap;
 };
+
+namespace sphb {
+
+void Prof::begin(int kid, cudaStream_t s) {
+  ++launches;
+  if (!on) return;
+  if (used == cap) {
+    const uint32_t ncap = cap ? cap * 2 : 1024;
+    Rec* nr = (Rec*)realloc(recs, (size_t)ncap * sizeof(Rec));
+    if (!nr) {
+      on = false;
+      return;
+    }
+    recs = nr, cap = ncap;
+  }
+  Rec& r = recs[used];
+  r.kid = kid;
+  if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) {
+    on = false;
+    return;
+  }
+  cudaEventRecord(r.a, s);
+  ++used;
+  open = true;
+}
+
+void Prof::end(cudaStream_t s) {
+  if (!open) return;
+  cudaEventRecord(recs[used - 1].b, s);
+  open = false;
+}
+
+}  // namespace sphb
 
 namespace {
 
@@ -156,7 +190,7 @@ int make_mc(sph_ctx* ctx, const mc_params* mp, McConst& m) {
 }
 
 int build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, cudaStream_t s) {
-  launch_build_grid(ctx->sc.grid, ctx->pg, (const float4*)pos, (const float4*)vel, n, ctx->scan, s, &ctx->launches);
+  launch_build_grid(ctx->sc.grid, ctx->pg, (const float4*)pos, (const float4*)vel, n, ctx->scan, s, &ctx->prof, false);
   ctx->grid_pos = pos;
   ctx->grid_vel = vel;
   ctx->grid_n = n;
@@ -228,6 +262,8 @@ int sph_destroy(sph_ctx* ctx) {
   free_grid(ctx->bg);
   cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->n_tris_dev);
   cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket);
+  sph_profile_enable(ctx, 0);
+  free(ctx->prof.recs);
   cudaFree(ctx->h_pos), cudaFree(ctx->h_vel), cudaFree(ctx->h_bpos), cudaFree(ctx->h_bvel), cudaFree(ctx->h_tris);
   delete ctx;
   return SPH_OK;
@@ -242,7 +278,43 @@ uint32_t sph_grid_dims(const sph_ctx* ctx, uint32_t dims_out[3]) {
   return ctx->sc.grid.C;
 }
 
-uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->launches : 0; }
+uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches : 0; }
+
+static const char* const kKernelNames[K_NUM_KERNELS] = {
+    "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
+    "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_boid_step",
+    "k_voxel_sdf", "k_mc_polygonise", "k_zero_u32"};
+
+const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
+
+int sph_profile_enable(sph_ctx* ctx, int enable) {
+  if (!ctx) return SPH_E_INVALID;
+  CK(cudaSetDevice(ctx->device));
+  Prof& pr = ctx->prof;
+  for (uint32_t i = 0; i < pr.used; ++i) cudaEventDestroy(pr.recs[i].a), cudaEventDestroy(pr.recs[i].b);
+  pr.used = 0;
+  for (int k = 0; k < K_NUM_KERNELS; ++k) pr.total_ms[k] = 0.0, pr.count[k] = 0;
+  pr.on = enable != 0;
+  return SPH_OK;
+}
+
+int sph_profile_read(sph_ctx* ctx, uint32_t kernel_id, uint64_t* launches_host, double* total_ms_host) {
+  if (!ctx || kernel_id >= K_NUM_KERNELS) return SPH_E_INVALID;
+  CK(cudaSetDevice(ctx->device));
+  Prof& pr = ctx->prof;
+  for (uint32_t i = 0; i < pr.used; ++i) {  // fold the pending event pairs into the totals
+    CK(cudaEventSynchronize(pr.recs[i].b));
+    float ms = 0.0f;
+    CK(cudaEventElapsedTime(&ms, pr.recs[i].a, pr.recs[i].b));
+    pr.total_ms[pr.recs[i].kid] += (double)ms;
+    pr.count[pr.recs[i].kid] += 1;
+    cudaEventDestroy(pr.recs[i].a), cudaEventDestroy(pr.recs[i].b);
+  }
+  pr.used = 0;
+  if (launches_host) *launches_host = pr.count[kernel_id];
+  if (total_ms_host) *total_ms_host = pr.total_ms[kernel_id];
+  return SPH_OK;
+}
 
 void sph_mc_table(int8_t* tri_host, uint8_t* ntri_host) { mc_table_host(tri_host, ntri_host); }
 
@@ -281,12 +353,12 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     int rc = set_boid_params(ctx, bp);
     if (rc != SPH_OK) return rc;
     launch_build_grid(ctx->bc.grid, ctx->bg, (const float4*)bpos, (const float4*)bvel, n_boid, ctx->scan, s,
-                      &ctx->launches);  // S7 / K14: Boid Space hash, same machinery as the particle grid
+                      &ctx->prof, true);  // S7 / K14: Boid Space hash, same machinery as the particle grid
   }
-  launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, s, &ctx->launches);
-  if (n_boid > 0) launch_boid_density(ctx->sc, ctx->pg, ctx->bg, n_boid, ctx->rho_bS, s, &ctx->launches);
+  launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, s, &ctx->prof);
+  if (n_boid > 0) launch_boid_density(ctx->sc, ctx->pg, ctx->bg, n_boid, ctx->rho_bS, s, &ctx->prof);
   launch_force_integrate(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS,
-                         ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, s, &ctx->launches);
+                         ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, s, &ctx->prof);
   ctx->grid_fresh = false;  // positions moved
   ctx->step_state = true;   // pg / rhoS still describe the step-start state (for boid_step)
   if (n_boid > 0) {
@@ -314,7 +386,7 @@ int boid_step(sph_ctx* ctx, const boid_params* bp, void* bpos, void* bvel, uint3
   if (memcmp(&keep, &ctx->bc.grid, sizeof(GridDesc)) != 0)
     return fail(ctx, SPH_E_STALE_GRID, "boid ranges / space changed since sph_step");
   launch_boid_step(ctx->sc, ctx->bc, ctx->pg, ctx->bg, ctx->grid_n, n_boid, ctx->rhoS, ctx->rho_bS, (float4*)bpos,
-                   (float4*)bvel, (float4*)dv_parts, s, &ctx->launches);
+                   (float4*)bvel, (float4*)dv_parts, s, &ctx->prof);
   ctx->boid_state = false;  // boids moved
   CK(cudaGetLastError());
   return SPH_OK;
@@ -328,7 +400,7 @@ int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi) {
   if (!phi) return fail(ctx, SPH_E_INVALID, "phi is NULL");
   if (!ctx->grid_fresh) return fail(ctx, SPH_E_STALE_GRID, "mc needs sph_build_grid on the current positions");
   CK(cudaSetDevice(ctx->device));
-  launch_voxel_sdf(ctx->sc, m, ctx->pg, phi, (cudaStream_t)stream, &ctx->launches);
+  launch_voxel_sdf(ctx->sc, m, ctx->pg, phi, (cudaStream_t)stream, &ctx->prof);
   CK(cudaGetLastError());
   return SPH_OK;
 }
@@ -342,7 +414,7 @@ int mc_polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, void* str
   if (!phi || (tri_capacity > 0 && !tris)) return fail(ctx, SPH_E_INVALID, "phi / tris is NULL");
   cudaStream_t s = (cudaStream_t)stream;
   CK(cudaSetDevice(ctx->device));
-  launch_mc_polygonise(m, phi, tris, tri_capacity, ctx->n_tris_dev, ctx->scan, s, &ctx->launches);
+  launch_mc_polygonise(m, phi, tris, tri_capacity, ctx->n_tris_dev, ctx->scan, s, &ctx->prof);
   if (n_tris_dev) CK(cudaMemcpyAsync(n_tris_dev, ctx->n_tris_dev, 4, cudaMemcpyDeviceToDevice, s));
   CK(cudaGetLastError());
   if (n_tris_host) {

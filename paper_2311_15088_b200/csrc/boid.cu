@@ -138,13 +138,14 @@ k_boid_step(SphConst c, BoidConst bc, const float4* __restrict__ posS, const flo
 
 void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                       uint32_t nb, const float* rhoS, const float* rho_bS, float4* bpos, float4* bvel,
-                      float4* dv_parts, cudaStream_t s, uint64_t* launches) {
+                      float4* dv_parts, cudaStream_t s, Prof* prof) {
   (void)n;
   if (nb == 0) return;
   const uint32_t warps_per_block = kThreads / 32;
+  prof->begin(K_BOID_STEP, s);
   k_boid_step<<<(nb + warps_per_block - 1) / warps_per_block, kThreads, 0, s>>>(
       c, bc, pg.posS, pg.velS, rhoS, pg.start, bg.posS, bg.velS, rho_bS, bg.start, bg.perm, nb, bpos, bvel, dv_parts);
-  ++*launches;
+  prof->end(s);
 }
 
 }  // namespace sphb

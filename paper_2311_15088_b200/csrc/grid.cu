@@ -116,21 +116,27 @@ __global__ void __launch_bounds__(kThreads) k_reorder(const uint32_t* __restrict
 uint32_t grid_scan_tiles(uint32_t C) { return (C + 1 + kScanTile - 1) / kScanTile; }
 
 void launch_build_grid(const GridDesc& g, const GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
-                       ScanState& scan, cudaStream_t s, uint64_t* launches) {
+                       ScanState& scan, cudaStream_t s, Prof* prof, bool boid_grid) {
   const uint32_t blocks = (n + kThreads - 1) / kThreads;
+  const int k0 = boid_grid ? K_BOID_HASH_COUNT : K_HASH_COUNT;
   if (n > 0) {
+    prof->begin(k0 + 0, s);
     k_hash_count<<<blocks, kThreads, 0, s>>>(g, pos, n, b.key, b.rank, b.count);
-    ++*launches;
+    prof->end(s);
   }
   const uint32_t tiles = grid_scan_tiles(g.C);
   scan.epoch += 1;
+  prof->begin(k0 + 1, s);
   k_scan_cells<<<tiles, kThreads, 0, s>>>(b.count, b.start, g.C, scan);
+  prof->end(s);
   scan.ticket_base += tiles;
-  ++*launches;
   if (n > 0) {
+    prof->begin(k0 + 2, s);
     k_scatter<<<blocks, kThreads, 0, s>>>(b.key, b.rank, b.start, n, b.slot_id);
+    prof->end(s);
+    prof->begin(k0 + 3, s);
     k_reorder<<<blocks, kThreads, 0, s>>>(b.key, b.start, b.slot_id, pos, vel, n, b.perm, b.posS, b.velS);
-    *launches += 2;
+    prof->end(s);
   }
 }
 

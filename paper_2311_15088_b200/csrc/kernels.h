@@ -33,6 +33,29 @@ struct McConst {
   int reach;            // ceil(R / h) particle cells (D:A-R)
 };
 
+// Kernel ids for the per-kernel timing that bench.py's roofline object is built from (sph_profile_*).
+enum KernelId {
+  K_HASH_COUNT = 0, K_SCAN_CELLS, K_SCATTER, K_REORDER,          // particle grid
+  K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
+  K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_BOID_STEP, K_VOXEL_SDF, K_MC_POLYGONISE, K_ZERO_U32,
+  K_NUM_KERNELS
+};
+
+// Launch bookkeeping: a counter always; when `on`, a CUDA event before and after every launch, recorded on
+// the launching stream (the kernels of one call are serialised on that stream anyway).
+struct Prof {
+  uint64_t launches;
+  bool on;
+  struct Rec { int kid; cudaEvent_t a, b; };
+  Rec* recs;
+  uint32_t used, cap;
+  bool open;
+  double total_ms[K_NUM_KERNELS];
+  uint64_t count[K_NUM_KERNELS];
+  void begin(int kid, cudaStream_t s);
+  void end(cudaStream_t s);
+};
+
 // Scratch of one grid (particles or boids).
 struct GridBuf {
   uint32_t* key;        // [n] cell of each point (caller order)
@@ -47,28 +70,28 @@ struct GridBuf {
 
 // grid.cu
 void launch_build_grid(const GridDesc& g, const GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
-                       ScanState& scan, cudaStream_t s, uint64_t* launches);
+                       ScanState& scan, cudaStream_t s, Prof* prof, bool boid_grid);
 uint32_t grid_scan_tiles(uint32_t C);
 // sph.cu
 void launch_density(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
-                    uint32_t* ncount_out, cudaStream_t s, uint64_t* launches);
+                    uint32_t* ncount_out, cudaStream_t s, Prof* prof);
 void launch_boid_density(const SphConst& c, const GridBuf& pg, const GridBuf& bg, uint32_t nb, float* rho_bS,
-                         cudaStream_t s, uint64_t* launches);
+                         cudaStream_t s, Prof* prof);
 void launch_force_integrate(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg,
                             uint32_t n, uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos,
                             float4* vel, float4* accel_out, uint32_t* touched_out, cudaStream_t s,
-                            uint64_t* launches);
+                            Prof* prof);
 // boid.cu
 void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                       uint32_t nb, const float* rhoS, const float* rho_bS, float4* bpos, float4* bvel,
-                      float4* dv_parts, cudaStream_t s, uint64_t* launches);
+                      float4* dv_parts, cudaStream_t s, Prof* prof);
 // mc.cu
 void upload_mc_tables();
 void mc_table_host(int8_t* tri, uint8_t* ntri);
 void launch_voxel_sdf(const SphConst& c, const McConst& m, const GridBuf& pg, float* phi, cudaStream_t s,
-                      uint64_t* launches);
+                      Prof* prof);
 void launch_mc_polygonise(const McConst& m, const float* phi, float* tris, uint32_t capacity, uint32_t* n_tris_dev,
-                          ScanState& scan, cudaStream_t s, uint64_t* launches);
+                          ScanState& scan, cudaStream_t s, Prof* prof);
 uint32_t mc_num_tiles(uint32_t G);
 
 }  // namespace sphb

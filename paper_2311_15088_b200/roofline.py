@@ -1,0 +1,68 @@
+"""Algorithmic bytes per kernel launch -- bookkeeping for bench.py.
+
+"Algorithmic" = the compulsory traffic of the method with SoA float4 state, every array touched once per
+pass: what a perfect implementation would have to move through HBM.  Bytes the implementation moves on top
+(scratch such as the arrival ranks, re-reads served by L2) are NOT counted, so achieved GB/s = these bytes /
+measured time is a lower bound on nothing and an upper bound on nothing: it is the roofline coordinate.
+
+N particles, C particle-grid cells, B boids, Cb boid-grid cells, G^3 voxel corners, T triangles.
+"""
+
+
+def kernel_bytes(n, c, nb, cb, g, t):
+    v = g ** 3
+    return {
+        # S1-S2: read pos 16, write key 4
+        "k_hash_count": 20 * n,
+        # S3: read count 4, write start 4 per cell
+        "k_scan_cells": 8 * c,
+        # S4: read key 4, pos 16, vel 16; write posS 16, velS 16, perm 4
+        "k_scatter": 0,        # implementation split of S4: its bytes are counted on k_reorder
+        "k_reorder": 72 * n,
+        "k_hash_count[boid grid]": 20 * nb,
+        "k_scan_cells[boid grid]": 8 * cb,
+        "k_scatter[boid grid]": 0,
+        "k_reorder[boid grid]": 72 * nb,
+        # S6: read posS 16 + cell table 8 per cell, write rho 4
+        "k_density": 20 * n + 8 * c,
+        # S7: read bpos 16, write rho_b 4 (the fluid it gathers is already counted)
+        "k_boid_density": 20 * nb,
+        # S8-S10: read posS 16, velS 16, rho 4, perm 4; write pos' 16, vel' 16
+        "k_force_integrate": 72 * n,
+        # S11-S13: read bpos, bvel 32, rho_b 4, perm 4; write 32
+        "k_boid_step": 72 * nb,
+        # S14: write phi 4 per corner; read posS 16 per particle and the cell table 8 per cell
+        "k_voxel_sdf": 4 * v + 16 * n + 8 * c,
+        # S15-S17: read phi 4 per corner, write 36 per triangle
+        "k_mc_polygonise": 4 * v + 36 * t,
+        "k_zero_u32": 4,
+    }
+
+
+SIM_KERNELS = ("k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]",
+               "k_scan_cells[boid grid]", "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density",
+               "k_boid_density", "k_force_integrate", "k_boid_step")
+MC_KERNELS = ("k_voxel_sdf", "k_mc_polygonise")
+
+
+def summarise(profile, n, c, nb, cb, g, t, peak_gbs):
+    """profile: {kernel: (launches, total_ms)}.  Returns (per-kernel rows, dominant kernel name).
+
+    Row: dict(kernel, launches, avg_us, share, bytes, gbs, frac).  share = fraction of the summed kernel time.
+    """
+    kb = kernel_bytes(n, c, nb, cb, g, t)
+    total = sum(ms for _, ms in profile.values()) or 1.0
+    rows = []
+    for name, (cnt, ms) in profile.items():
+        avg_ms = ms / max(cnt, 1)
+        b = kb.get(name, 0)
+        gbs = b / (avg_ms * 1e-3) / 1e9 if avg_ms > 0 else 0.0
+        rows.append(dict(kernel=name, launches=cnt, avg_us=avg_ms * 1e3, share=ms / total, bytes=b, gbs=gbs,
+                         frac=gbs / peak_gbs))
+    rows.sort(key=lambda r: -r["share"])
+    return rows, (rows[0]["kernel"] if rows else None)
+
+
+def pass_bytes(names, n, c, nb, cb, g, t):
+    kb = kernel_bytes(n, c, nb, cb, g, t)
+    return sum(kb[k] for k in names)
