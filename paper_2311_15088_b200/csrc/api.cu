@@ -22,6 +22,8 @@ struct sph_ctx {
   float* rhoS;
   float* rho_bS;
   float* phi;   // [Gmax^3]
+  uint32_t* sdf_first;  // corner partition tables of the surface pass (SdfPlan::first)
+  uint32_t sdf_first_cap;
   uint32_t* n_tris_dev;
   ScanState scan;
   uint32_t max_tiles;
@@ -125,6 +127,14 @@ int alloc_grid(sph_ctx* ctx, GridBuf& b, uint32_t n, uint32_t C) {
   CK(cudaMalloc(&b.perm, nn * 4));
   CK(cudaMalloc(&b.posS, nn * 16));
   CK(cudaMalloc(&b.velS, nn * 16));
+  CK(cudaMalloc(&b.aabb, 12 * 4));
+  CK(cudaMalloc(&b.box_part, ((nn + 255) / 256) * 6 * 4));
+  {
+    const uint32_t empty[12] = {~0u, ~0u, ~0u, 0u, 0u, 0u, ~0u, ~0u, ~0u, 0u, 0u, 0u};
+    CK(cudaMemcpy(b.aabb, empty, sizeof(empty), cudaMemcpyHostToDevice));
+  }
+  b.slot = 0;
+  b.aabb_now = b.aabb;
   CK(cudaMemset(b.count, 0, ((size_t)C + 8) * 4));
   CK(cudaMemset(b.start, 0, ((size_t)C + 9) * 4));
   return SPH_OK;
@@ -132,7 +142,7 @@ int alloc_grid(sph_ctx* ctx, GridBuf& b, uint32_t n, uint32_t C) {
 
 void free_grid(GridBuf& b) {
   cudaFree(b.key), cudaFree(b.rank), cudaFree(b.count), cudaFree(b.start);
-  cudaFree(b.slot_id), cudaFree(b.perm), cudaFree(b.posS), cudaFree(b.velS);
+  cudaFree(b.slot_id), cudaFree(b.perm), cudaFree(b.posS), cudaFree(b.velS), cudaFree(b.aabb), cudaFree(b.box_part);
   memset(&b, 0, sizeof(b));
 }
 
@@ -177,6 +187,7 @@ int make_mc(sph_ctx* ctx, const mc_params* mp, McConst& m) {
   if (mp->n_point_per_axis > ctx->p.max_mc_points_per_axis)
     return fail(ctx, SPH_E_INVALID, "n_point_per_axis exceeds max_mc_points_per_axis");
   if (!(mp->radius > 0.0f)) return fail(ctx, SPH_E_INVALID, "mc radius must be positive");
+  if (!(mp->spacing > 0.0f)) return fail(ctx, SPH_E_INVALID, "mc spacing must be positive");
   for (int a = 0; a < 3; ++a) m.origin[a] = mp->origin[a];
   m.spacing = mp->spacing;
   m.G = mp->n_point_per_axis;
@@ -239,7 +250,10 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   const size_t G = p->max_mc_points_per_axis;
   if (cudaMalloc(&ctx->rhoS, nn * 4) != cudaSuccess || cudaMalloc(&ctx->rho_bS, nb * 4) != cudaSuccess ||
       cudaMalloc(&ctx->phi, std::max<size_t>(G * G * G, 1) * 4) != cudaSuccess ||
-      cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess || cudaMalloc(&ctx->scan.ticket, 4) != cudaSuccess)
+      cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess ||
+      cudaMalloc(&ctx->sdf_first, (size_t)(ctx->sdf_first_cap = (uint32_t)(sc.grid.dim[0] + sc.grid.dim[1] +
+                                                                          sc.grid.dim[2] + 3 * (2 * 16 + 3))) * 4) !=
+          cudaSuccess || cudaMalloc(&ctx->scan.ticket, 4) != cudaSuccess)
     return bail(SPH_E_CUDA);
   ctx->max_tiles = std::max(std::max(grid_scan_tiles(sc.grid.C), grid_scan_tiles(ctx->boid_cells_cap)),
                             std::max(mc_num_tiles((uint32_t)G), 1u));
@@ -260,7 +274,7 @@ int sph_destroy(sph_ctx* ctx) {
   cudaSetDevice(ctx->device);
   free_grid(ctx->pg);
   free_grid(ctx->bg);
-  cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->n_tris_dev);
+  cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->n_tris_dev), cudaFree(ctx->sdf_first);
   cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket);
   sph_profile_enable(ctx, 0);
   free(ctx->prof.recs);
@@ -283,7 +297,7 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_boid_step",
-    "k_voxel_sdf", "k_mc_polygonise", "k_zero_u32"};
+    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_mc_polygonise", "k_zero_u32"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -400,7 +414,7 @@ int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi) {
   if (!phi) return fail(ctx, SPH_E_INVALID, "phi is NULL");
   if (!ctx->grid_fresh) return fail(ctx, SPH_E_STALE_GRID, "mc needs sph_build_grid on the current positions");
   CK(cudaSetDevice(ctx->device));
-  launch_voxel_sdf(ctx->sc, m, ctx->pg, phi, (cudaStream_t)stream, &ctx->prof);
+  launch_voxel_sdf(ctx->sc, m, ctx->pg, ctx->sdf_first, ctx->sdf_first_cap, phi, (cudaStream_t)stream, &ctx->prof);
   CK(cudaGetLastError());
   return SPH_OK;
 }

@@ -13,24 +13,81 @@ constexpr int kScanTile = kThreads * kScanItems;  // 2048 cells per tile
 // S1 + S2 (P:426-432 set_particle_count): key = hash(get_cell(p)); rank = atomicAdd(count[key], 1).
 __global__ void __launch_bounds__(kThreads) k_hash_count(GridDesc g, const float4* __restrict__ pos, uint32_t n,
                                                          uint32_t* __restrict__ key, uint32_t* __restrict__ rank,
-                                                         uint32_t* __restrict__ count) {
+                                                         uint32_t* __restrict__ count, uint32_t* __restrict__ box_part) {
   const uint32_t i = blockIdx.x * kThreads + threadIdx.x;
-  if (i >= n) return;
-  const float4 p = __ldg(pos + i);
-  const int cx = cell_coord(p.x, g.lo[0], g.cell, g.dim[0]);
-  const int cy = cell_coord(p.y, g.lo[1], g.cell, g.dim[1]);
-  const int cz = cell_coord(p.z, g.lo[2], g.cell, g.dim[2]);
-  const uint32_t k = cell_hash(g, cx, cy, cz);
-  key[i] = k;
-  rank[i] = atomicAdd(count + k, 1u);
+  const bool in = i < n;
+  const float4 p = __ldg(pos + (in ? i : n - 1));
+  if (in) {
+    const int cx = cell_coord(p.x, g.lo[0], g.cell, g.dim[0]);
+    const int cy = cell_coord(p.y, g.lo[1], g.cell, g.dim[1]);
+    const int cz = cell_coord(p.z, g.lo[2], g.cell, g.dim[2]);
+    const uint32_t k = cell_hash(g, cx, cy, cz);
+    key[i] = k;
+    rank[i] = atomicAdd(count + k, 1u);
+  }
+  // bounding box of the points (order-preserving uint encoding), used by the surface pass to skip corners that
+  // are further than R from every particle: warp min / max, block min / max through shared memory, one partial
+  // per block; the scan kernel folds the partials (no same-address atomics from 10^4 blocks)
+  __shared__ uint32_t s_box[kThreads / 32][6];
+  float lo[3] = {p.x, p.y, p.z}, hi[3] = {p.x, p.y, p.z};
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+      hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+    }
+  if ((threadIdx.x & 31u) == 0) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      s_box[threadIdx.x >> 5][a] = encode_ordered(lo[a]);
+      s_box[threadIdx.x >> 5][3 + a] = encode_ordered(hi[a]);
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    uint32_t v = s_box[0][threadIdx.x];
+#pragma unroll
+    for (int w = 1; w < kThreads / 32; ++w)
+      v = threadIdx.x < 3 ? min(v, s_box[w][threadIdx.x]) : max(v, s_box[w][threadIdx.x]);
+    box_part[blockIdx.x * 6 + threadIdx.x] = v;
+  }
 }
 
 // S3 (D:A-OFFSET): exclusive scan of the histogram in ONE pass -- block-local scan plus
 // decoupled look-back over tile aggregates -- instead of the paper's up-sweep / down-sweep.  Scans C+1
 // entries (entry C counts 0) so that start[C] = total, and clears the histogram for the next build.
 __global__ void __launch_bounds__(kThreads) k_scan_cells(uint32_t* __restrict__ count, uint32_t* __restrict__ start,
-                                                         uint32_t C, ScanState st) {
+                                                         uint32_t C, ScanState st,
+                                                         const uint32_t* __restrict__ box_part, uint32_t n_parts,
+                                                         uint32_t* __restrict__ aabb, uint32_t* __restrict__ aabb_next) {
   __shared__ uint32_t s_scan[33];
+  if (blockIdx.x == 0 && threadIdx.x < 6) aabb_next[threadIdx.x] = threadIdx.x < 3 ? 0xffffffffu : 0u;  // empty box
+  if (threadIdx.x >= 32 && threadIdx.x < 64) {  // warp 1 folds this block's share of the bounding-box partials
+    const uint32_t lane = threadIdx.x - 32;
+    uint32_t v[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
+    for (uint32_t q = blockIdx.x + lane * gridDim.x; q < n_parts; q += 32 * gridDim.x) {
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        v[a] = min(v[a], __ldg(box_part + 6 * q + a));
+        v[3 + a] = max(v[3 + a], __ldg(box_part + 6 * q + 3 + a));
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        v[a] = min(v[a], __shfl_xor_sync(0xffffffffu, v[a], o));
+        v[3 + a] = max(v[3 + a], __shfl_xor_sync(0xffffffffu, v[3 + a], o));
+      }
+    if (lane == 0 && blockIdx.x < n_parts) {
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        atomicMin(aabb + a, v[a]);
+        atomicMax(aabb + 3 + a, v[3 + a]);
+      }
+    }
+  }
   __shared__ uint32_t s_tile, s_base;
   if (threadIdx.x == 0) s_tile = atomicAdd(st.ticket, 1u) - st.ticket_base;
   __syncthreads();
@@ -115,19 +172,21 @@ __global__ void __launch_bounds__(kThreads) k_reorder(const uint32_t* __restrict
 
 uint32_t grid_scan_tiles(uint32_t C) { return (C + 1 + kScanTile - 1) / kScanTile; }
 
-void launch_build_grid(const GridDesc& g, const GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
+void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
                        ScanState& scan, cudaStream_t s, Prof* prof, bool boid_grid) {
   const uint32_t blocks = (n + kThreads - 1) / kThreads;
   const int k0 = boid_grid ? K_BOID_HASH_COUNT : K_HASH_COUNT;
   if (n > 0) {
     prof->begin(k0 + 0, s);
-    k_hash_count<<<blocks, kThreads, 0, s>>>(g, pos, n, b.key, b.rank, b.count);
+    k_hash_count<<<blocks, kThreads, 0, s>>>(g, pos, n, b.key, b.rank, b.count, b.box_part);
     prof->end(s);
   }
   const uint32_t tiles = grid_scan_tiles(g.C);
   scan.epoch += 1;
   prof->begin(k0 + 1, s);
-  k_scan_cells<<<tiles, kThreads, 0, s>>>(b.count, b.start, g.C, scan);
+  // the scan also empties the OTHER bounding-box slot, which the next build fills
+  k_scan_cells<<<tiles, kThreads, 0, s>>>(b.count, b.start, g.C, scan, b.box_part, n > 0 ? blocks : 0u,
+                                          b.aabb + 6 * b.slot, b.aabb + 6 * (b.slot ^ 1));
   prof->end(s);
   scan.ticket_base += tiles;
   if (n > 0) {
@@ -138,6 +197,8 @@ void launch_build_grid(const GridDesc& g, const GridBuf& b, const float4* pos, c
     k_reorder<<<blocks, kThreads, 0, s>>>(b.key, b.start, b.slot_id, pos, vel, n, b.perm, b.posS, b.velS);
     prof->end(s);
   }
+  b.aabb_now = b.aabb + 6 * b.slot;
+  b.slot ^= 1;
 }
 
 }  // namespace sphb

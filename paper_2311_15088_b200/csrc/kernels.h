@@ -37,7 +37,8 @@ struct McConst {
 enum KernelId {
   K_HASH_COUNT = 0, K_SCAN_CELLS, K_SCATTER, K_REORDER,          // particle grid
   K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
-  K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_BOID_STEP, K_VOXEL_SDF, K_MC_POLYGONISE, K_ZERO_U32,
+  K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_BOID_STEP, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
+  K_MC_POLYGONISE, K_ZERO_U32,
   K_NUM_KERNELS
 };
 
@@ -66,10 +67,22 @@ struct GridBuf {
   uint32_t* perm;       // [n] sorted slot -> id, ascending id inside a cell (D:A-SORT)
   float4* posS;         // [n] cell-sorted copies
   float4* velS;
+  uint32_t* aabb;       // [2][6] bounding box of the points (min xyz, max xyz; order-preserving encoding), two slots
+  uint32_t* box_part;   // [ceil(n/256)][6] per-block partial bounding boxes of the hash kernel
+  int slot;             // slot the NEXT build fills (the scan of each build empties the other one)
+  const uint32_t* aabb_now;  // slot of the last build
+};
+
+// Corner partition of the voxel grid by particle cell (mc.cu, k_voxel_sdf_groups).
+struct SdfPlan {
+  int nv[3];            // virtual cells per axis: dim + 2 reach + 2
+  int gsz[3];           // group size in virtual cells
+  int ng[3];            // groups per axis
+  uint32_t* first[3];   // [nv+1] first corner index of each virtual cell
 };
 
 // grid.cu
-void launch_build_grid(const GridDesc& g, const GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
+void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
                        ScanState& scan, cudaStream_t s, Prof* prof, bool boid_grid);
 uint32_t grid_scan_tiles(uint32_t C);
 // sph.cu
@@ -88,8 +101,8 @@ void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg,
 // mc.cu
 void upload_mc_tables();
 void mc_table_host(int8_t* tri, uint8_t* ntri);
-void launch_voxel_sdf(const SphConst& c, const McConst& m, const GridBuf& pg, float* phi, cudaStream_t s,
-                      Prof* prof);
+void launch_voxel_sdf(const SphConst& c, const McConst& m, const GridBuf& pg, uint32_t* sdf_first,
+                      uint32_t sdf_first_cap, float* phi, cudaStream_t s, Prof* prof);
 void launch_mc_polygonise(const McConst& m, const float* phi, float* tris, uint32_t capacity, uint32_t* n_tris_dev,
                           ScanState& scan, cudaStream_t s, Prof* prof);
 uint32_t mc_num_tiles(uint32_t G);
