@@ -33,6 +33,8 @@ def kernel_bytes(n, c, nb, cb, g, t):
         "k_boid_step": 72 * nb,
         # S14: write phi 4 per corner; read posS 16 per particle and the cell table 8 per cell
         "k_voxel_sdf": 4 * v + 16 * n + 8 * c,
+        "k_voxel_sdf_groups": 4 * v + 16 * n + 8 * c,   # the warp-per-cell-group variant of the same row
+        "k_sdf_axis_tables": 0,                         # helper of S14 (axis partition tables): bytes counted above
         # S15-S17: read phi 4 per corner, write 36 per triangle
         "k_mc_polygonise": 4 * v + 36 * t,
         "k_zero_u32": 4,
@@ -42,7 +44,7 @@ def kernel_bytes(n, c, nb, cb, g, t):
 SIM_KERNELS = ("k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]",
                "k_scan_cells[boid grid]", "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density",
                "k_boid_density", "k_force_integrate", "k_boid_step")
-MC_KERNELS = ("k_voxel_sdf", "k_mc_polygonise")
+MC_KERNELS = ("k_voxel_sdf", "k_mc_polygonise")  # one of k_voxel_sdf / k_voxel_sdf_groups runs per pass
 
 
 def summarise(profile, n, c, nb, cb, g, t, peak_gbs):
