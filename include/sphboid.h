@@ -112,6 +112,11 @@ int boid_step(sph_ctx* ctx, const boid_params* bp /* host */, void* bpos, void* 
  * positions to mesh) else SPH_E_STALE_GRID.  phi[G^3]. */
 int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, float* phi);
 
+/* S14 has three kernels that compute the same phi: 1 = one thread per corner, 2 = a warp per
+ * group of particle cells, 3 = a warp per block of 4x4x2 corners with a filtered candidate list.  0 (default) picks
+ * by a cost model from the voxel spacing; the others force one (tests, A/B measurements). */
+int mc_set_sdf_variant(sph_ctx* ctx, int variant);
+
 /* S15-S17: marching cubes on a given phi[G^3] (Listing 10-11, Eq. 51): case per cube,
  * triangle count, device-wide exclusive scan, ordered emit (cube-major, then table order; D:A-APPEND).
  * tris = tri_capacity * 9 floats (3 vertices x xyz).  *n_tris_host (host, optional) gets the REQUIRED

@@ -34,6 +34,7 @@ def kernel_bytes(n, c, nb, cb, g, t):
         # S14: write phi 4 per corner; read posS 16 per particle and the cell table 8 per cell
         "k_voxel_sdf": 4 * v + 16 * n + 8 * c,
         "k_voxel_sdf_groups": 4 * v + 16 * n + 8 * c,   # the warp-per-cell-group variant of the same row
+        "k_voxel_sdf_blocks": 4 * v + 16 * n + 8 * c,   # the warp-per-corner-block variant of the same row
         "k_sdf_axis_tables": 0,                         # helper of S14 (axis partition tables): bytes counted above
         # S15-S17: read phi 4 per corner, write 36 per triangle
         "k_mc_polygonise": 4 * v + 36 * t,
