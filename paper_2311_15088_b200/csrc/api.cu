@@ -22,6 +22,7 @@ struct sph_ctx {
   float* rhoS;
   float* rho_bS;
   float* phi;   // [Gmax^3]
+  uint32_t* mc_bits;  // [ceil(Gmax/32) * Gmax^2] corner sign bits of the surface pass
   uint32_t* sdf_first;  // corner partition tables of the surface pass (SdfPlan::first)
   uint32_t sdf_first_cap;
   int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = cell groups, 3 = corner blocks (mc_set_sdf_variant)
@@ -251,6 +252,7 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   const size_t G = p->max_mc_points_per_axis;
   if (cudaMalloc(&ctx->rhoS, nn * 4) != cudaSuccess || cudaMalloc(&ctx->rho_bS, nb * 4) != cudaSuccess ||
       cudaMalloc(&ctx->phi, std::max<size_t>(G * G * G, 1) * 4) != cudaSuccess ||
+      cudaMalloc(&ctx->mc_bits, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4) != cudaSuccess ||
       cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess ||
       cudaMalloc(&ctx->sdf_first, (size_t)(ctx->sdf_first_cap = (uint32_t)(sc.grid.dim[0] + sc.grid.dim[1] +
                                                                           sc.grid.dim[2] + 3 * (2 * 16 + 3))) * 4) !=
@@ -275,7 +277,7 @@ int sph_destroy(sph_ctx* ctx) {
   cudaSetDevice(ctx->device);
   free_grid(ctx->pg);
   free_grid(ctx->bg);
-  cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->n_tris_dev), cudaFree(ctx->sdf_first);
+  cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->sdf_first);
   cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket);
   sph_profile_enable(ctx, 0);
   free(ctx->prof.recs);
@@ -298,7 +300,7 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_boid_step",
-    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_mc_polygonise", "k_zero_u32"};
+    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_mc_signs", "k_mc_polygonise", "k_zero_u32"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -437,7 +439,7 @@ int mc_polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, void* str
   if (!phi || (tri_capacity > 0 && !tris)) return fail(ctx, SPH_E_INVALID, "phi / tris is NULL");
   cudaStream_t s = (cudaStream_t)stream;
   CK(cudaSetDevice(ctx->device));
-  launch_mc_polygonise(m, phi, tris, tri_capacity, ctx->n_tris_dev, ctx->scan, s, &ctx->prof);
+  launch_mc_polygonise(m, phi, ctx->mc_bits, tris, tri_capacity, ctx->n_tris_dev, ctx->scan, s, &ctx->prof);
   if (n_tris_dev) CK(cudaMemcpyAsync(n_tris_dev, ctx->n_tris_dev, 4, cudaMemcpyDeviceToDevice, s));
   CK(cudaGetLastError());
   if (n_tris_host) {

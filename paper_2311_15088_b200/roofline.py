@@ -37,7 +37,8 @@ def kernel_bytes(n, c, nb, cb, g, t):
         "k_voxel_sdf_blocks": 4 * v + 16 * n + 8 * c,   # the warp-per-corner-block variant of the same row
         "k_sdf_axis_tables": 0,                         # helper of S14 (axis partition tables): bytes counted above
         # S15-S17: read phi 4 per corner, write 36 per triangle
-        "k_mc_polygonise": 4 * v + 36 * t,
+        "k_mc_signs": 4 * v,                            # S15 first half: read phi once -> 1 bit per corner
+        "k_mc_polygonise": 36 * t,                      # S15 second half - S17 on the bit field (G^3 / 8 bytes: < 1 %)
         "k_zero_u32": 4,
     }
 
@@ -45,7 +46,7 @@ def kernel_bytes(n, c, nb, cb, g, t):
 SIM_KERNELS = ("k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]",
                "k_scan_cells[boid grid]", "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density",
                "k_boid_density", "k_force_integrate", "k_boid_step")
-MC_KERNELS = ("k_voxel_sdf", "k_mc_polygonise")  # one of k_voxel_sdf / k_voxel_sdf_groups runs per pass
+MC_KERNELS = ("k_voxel_sdf", "k_mc_signs", "k_mc_polygonise")  # one of k_voxel_sdf / k_voxel_sdf_groups runs per pass
 
 
 def summarise(profile, n, c, nb, cb, g, t, peak_gbs):
