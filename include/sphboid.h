@@ -112,9 +112,10 @@ int boid_step(sph_ctx* ctx, const boid_params* bp /* host */, void* bpos, void* 
  * positions to mesh) else SPH_E_STALE_GRID.  phi[G^3]. */
 int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, float* phi);
 
-/* S14 has three kernels that compute the same phi: 1 = one thread per corner, 2 = a warp per
- * group of particle cells, 3 = a warp per block of 4x4x2 corners with a filtered candidate list.  0 (default) picks
- * by a cost model from the voxel spacing; the others force one (tests, A/B measurements). */
+/* S14 has four kernels that compute the same phi: 1 = one thread per corner, 2 = a warp per
+ * group of particle cells, 3 = a warp per block of 4x4x2 corners with a filtered candidate list, 4 = a warp per tile
+ * of 8x8x4 corners, 2x2x2 corners per lane, with per-lane candidate lists.  0 (default) picks by a cost model from the
+ * voxel spacing; the others force one (tests, A/B measurements). */
 int mc_set_sdf_variant(sph_ctx* ctx, int variant);
 
 /* S15-S17: marching cubes on a given phi[G^3] (Listing 10-11, Eq. 51): case per cube,

@@ -25,7 +25,7 @@ struct sph_ctx {
   uint32_t* mc_bits;  // [ceil(Gmax/32) * Gmax^2] corner sign bits of the surface pass
   uint32_t* sdf_first;  // corner partition tables of the surface pass (SdfPlan::first)
   uint32_t sdf_first_cap;
-  int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = cell groups, 3 = corner blocks (mc_set_sdf_variant)
+  int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = cell groups, 3 = corner blocks, 4 = corner tiles (mc_set_sdf_variant)
   uint32_t* n_tris_dev;
   ScanState scan;
   uint32_t max_tiles;
@@ -300,7 +300,7 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_boid_step",
-    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_mc_signs", "k_mc_polygonise", "k_zero_u32"};
+    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_mc_signs", "k_mc_polygonise", "k_zero_u32"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -425,7 +425,7 @@ int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi) {
 
 int mc_set_sdf_variant(sph_ctx* ctx, int variant) {
   if (!ctx) return SPH_E_INVALID;
-  if (variant < 0 || variant > 3) return fail(ctx, SPH_E_INVALID, "sdf variant must be 0..3");
+  if (variant < 0 || variant > 4) return fail(ctx, SPH_E_INVALID, "sdf variant must be 0..4");
   ctx->sdf_variant = variant;
   return SPH_OK;
 }

@@ -38,7 +38,7 @@ enum KernelId {
   K_HASH_COUNT = 0, K_SCAN_CELLS, K_SCATTER, K_REORDER,          // particle grid
   K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
   K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_BOID_STEP, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
-  K_VOXEL_SDF_BLOCKS, K_MC_SIGNS, K_MC_POLYGONISE, K_ZERO_U32,
+  K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_MC_SIGNS, K_MC_POLYGONISE, K_ZERO_U32,
   K_NUM_KERNELS
 };
 

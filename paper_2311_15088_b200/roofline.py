@@ -35,6 +35,7 @@ def kernel_bytes(n, c, nb, cb, g, t):
         "k_voxel_sdf": 4 * v + 16 * n + 8 * c,
         "k_voxel_sdf_groups": 4 * v + 16 * n + 8 * c,   # the warp-per-cell-group variant of the same row
         "k_voxel_sdf_blocks": 4 * v + 16 * n + 8 * c,   # the warp-per-corner-block variant of the same row
+        "k_voxel_sdf_tiles": 4 * v + 16 * n + 8 * c,    # the 2x2x2-corners-per-lane tile variant of the same row
         "k_sdf_axis_tables": 0,                         # helper of S14 (axis partition tables): bytes counted above
         # S15-S17: read phi 4 per corner, write 36 per triangle
         "k_mc_signs": 4 * v,                            # S15 first half: read phi once -> 1 bit per corner
