@@ -177,6 +177,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--force-variant", type=int, default=0, help="A/B: 0 = stored neighbour masks (default), 1 = grid walk")
+    ap.add_argument("--sdf-variant", type=int, default=0, help="A/B: 0 = cost model (default), 1-4 force one S14 kernel")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args, args.config)
@@ -201,6 +203,10 @@ def main():
     peak, peak_kind = measured_peak()
 
     fr = Frame(cfg, device=dev)
+    if args.force_variant:
+        B.sph_set_force_variant(fr.ctx, args.force_variant)
+    if args.sdf_variant:
+        B.mc_set_sdf_variant(fr.ctx, args.sdf_variant)
     G = fr.G
     _, C = B.sph_grid_dims(fr.ctx)
     for _ in range(args.warmup):

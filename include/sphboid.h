@@ -107,6 +107,11 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
 int boid_step(sph_ctx* ctx, const boid_params* bp /* host */, void* bpos, void* bvel, uint32_t n_boid,
               void* stream, void* dv_parts);
 
+/* S8 has two kernels that compute the same forces: 0 (default) = the density pass stores each
+ * particle's neighbour list (the paper's section 9 design) and the force pass reads it; 1 = the force pass
+ * walks the 27 cells again.  Tests and A/B measurements force one. */
+int sph_set_force_variant(sph_ctx* ctx, int variant);
+
 /* S14: voxel signed distance phi(x) = |x - xbar| - rbar, xbar the kernel-weighted mean neighbour position
  * (Eq. 48-50, Listing 9; D:A-PHI, D:A-PHI0).  Needs a current grid (sph_build_grid on the
  * positions to mesh) else SPH_E_STALE_GRID.  phi[G^3]. */

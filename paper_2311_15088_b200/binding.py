@@ -75,6 +75,7 @@ def lib():
         L.boid_step.argtypes = [_vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.mc_voxel_sdf.argtypes = [_vp, _vp, _vp, _vp]
         L.mc_set_sdf_variant.argtypes = [_vp, C.c_int]
+        L.sph_set_force_variant.argtypes = [_vp, C.c_int]
         L.mc_polygonise.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.mc_extract.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp]
         L.sph_simulate_host.argtypes = [_vp, _vp, _vp, _u32, _vp, _vp, _u32, _vp, _u32, _vp, _vp, _u32, _vp]
@@ -91,7 +92,7 @@ def lib():
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "mc_voxel_sdf", "mc_set_sdf_variant", "mc_polygonise", "mc_extract", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "mc_polygonise", "mc_extract", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
            "sph_profile_read", "sph_kernel_name"]
 
 
@@ -205,6 +206,10 @@ def boid_step(ctx, boid, bpos, bvel, stream=None, dv_parts=None):
 def mc_voxel_sdf(ctx, mc, phi, stream=None):
     m = _fill(McParams, mc)
     return _check(ctx, lib().mc_voxel_sdf(ctx, C.byref(m), _stream(stream), _ptr(phi)))
+
+
+def sph_set_force_variant(ctx, variant):
+    return _check(ctx, lib().sph_set_force_variant(ctx, int(variant)))
 
 
 def mc_set_sdf_variant(ctx, variant):

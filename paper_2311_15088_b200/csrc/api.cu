@@ -25,6 +25,8 @@ struct sph_ctx {
   uint32_t* mc_bits;  // [ceil(Gmax/32) * Gmax^2] corner sign bits of the surface pass
   uint32_t* sdf_first;  // corner partition tables of the surface pass (SdfPlan::first)
   uint32_t sdf_first_cap;
+  NbrList nbr;           // stored neighbour list of the last sph_step
+  int force_variant;     // 0 = stored neighbour list (k_force_list), 1 = grid walk (k_force_integrate)
   int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = cell groups, 3 = corner blocks, 4 = corner tiles (mc_set_sdf_variant)
   uint32_t* n_tris_dev;
   ScanState scan;
@@ -253,7 +255,8 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   if (cudaMalloc(&ctx->rhoS, nn * 4) != cudaSuccess || cudaMalloc(&ctx->rho_bS, nb * 4) != cudaSuccess ||
       cudaMalloc(&ctx->phi, std::max<size_t>(G * G * G, 1) * 4) != cudaSuccess ||
       cudaMalloc(&ctx->mc_bits, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4) != cudaSuccess ||
-      cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess ||
+      cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess || cudaMalloc(&ctx->nbr.cnt, nn * 2) != cudaSuccess ||
+      cudaMalloc(&ctx->nbr.list, (size_t)nbr_rows() * (ctx->nbr.stride = (uint32_t)((nn + 63) & ~(size_t)63)) * 2) != cudaSuccess ||
       cudaMalloc(&ctx->sdf_first, (size_t)(ctx->sdf_first_cap = (uint32_t)(sc.grid.dim[0] + sc.grid.dim[1] +
                                                                           sc.grid.dim[2] + 3 * (2 * 16 + 3))) * 4) !=
           cudaSuccess || cudaMalloc(&ctx->scan.ticket, 4) != cudaSuccess)
@@ -277,7 +280,7 @@ int sph_destroy(sph_ctx* ctx) {
   cudaSetDevice(ctx->device);
   free_grid(ctx->pg);
   free_grid(ctx->bg);
-  cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->sdf_first);
+  cudaFree(ctx->nbr.list), cudaFree(ctx->nbr.cnt), cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->sdf_first);
   cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket);
   sph_profile_enable(ctx, 0);
   free(ctx->prof.recs);
@@ -299,7 +302,7 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
-    "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_boid_step",
+    "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step",
     "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_mc_signs", "k_mc_polygonise", "k_zero_u32"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
@@ -372,10 +375,11 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     launch_build_grid(ctx->bc.grid, ctx->bg, (const float4*)bpos, (const float4*)bvel, n_boid, ctx->scan, s,
                       &ctx->prof, true);  // S7 / K14: Boid Space hash, same machinery as the particle grid
   }
-  launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, s, &ctx->prof);
+  const NbrList* nl = ctx->force_variant == 0 ? &ctx->nbr : nullptr;
+  launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, nl, s, &ctx->prof);
   if (n_boid > 0) launch_boid_density(ctx->sc, ctx->pg, ctx->bg, n_boid, ctx->rho_bS, s, &ctx->prof);
   launch_force_integrate(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS,
-                         ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, s, &ctx->prof);
+                         ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, nl, s, &ctx->prof);
   ctx->grid_fresh = false;  // positions moved
   ctx->step_state = true;   // pg / rhoS still describe the step-start state (for boid_step)
   if (n_boid > 0) {
@@ -427,6 +431,13 @@ int mc_set_sdf_variant(sph_ctx* ctx, int variant) {
   if (!ctx) return SPH_E_INVALID;
   if (variant < 0 || variant > 4) return fail(ctx, SPH_E_INVALID, "sdf variant must be 0..4");
   ctx->sdf_variant = variant;
+  return SPH_OK;
+}
+
+int sph_set_force_variant(sph_ctx* ctx, int variant) {
+  if (!ctx) return SPH_E_INVALID;
+  if (variant < 0 || variant > 1) return fail(ctx, SPH_E_INVALID, "force variant must be 0 or 1");
+  ctx->force_variant = variant;
   return SPH_OK;
 }
 

@@ -37,7 +37,7 @@ struct McConst {
 enum KernelId {
   K_HASH_COUNT = 0, K_SCAN_CELLS, K_SCATTER, K_REORDER,          // particle grid
   K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
-  K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_BOID_STEP, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
+  K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
   K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_MC_SIGNS, K_MC_POLYGONISE, K_ZERO_U32,
   K_NUM_KERNELS
 };
@@ -73,6 +73,13 @@ struct GridBuf {
   const uint32_t* aabb_now;  // slot of the last build
 };
 
+// Stored neighbour list (sph.cu): rows list[k * stride + i] of 16-bit entries, cnt[i] entries per sorted particle i.
+struct NbrList {
+  uint16_t* list;       // [nbr_rows() * stride]
+  uint16_t* cnt;        // [n]
+  uint32_t stride;      // elements between rows, a multiple of 64
+};
+
 // Corner partition of the voxel grid by particle cell (mc.cu, k_voxel_sdf_groups).
 struct SdfPlan {
   int nv[3];            // virtual cells per axis: dim + 2 reach + 2
@@ -87,13 +94,14 @@ void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const f
 uint32_t grid_scan_tiles(uint32_t C);
 // sph.cu
 void launch_density(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
-                    uint32_t* ncount_out, cudaStream_t s, Prof* prof);
+                    uint32_t* ncount_out, const NbrList* nl, cudaStream_t s, Prof* prof);
+uint32_t nbr_rows();
 void launch_boid_density(const SphConst& c, const GridBuf& pg, const GridBuf& bg, uint32_t nb, float* rho_bS,
                          cudaStream_t s, Prof* prof);
 void launch_force_integrate(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg,
                             uint32_t n, uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos,
-                            float4* vel, float4* accel_out, uint32_t* touched_out, cudaStream_t s,
-                            Prof* prof);
+                            float4* vel, float4* accel_out, uint32_t* touched_out, const NbrList* nl,
+                            cudaStream_t s, Prof* prof);
 // boid.cu
 void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                       uint32_t nb, const float* rhoS, const float* rho_bS, float4* bpos, float4* bvel,

@@ -29,6 +29,7 @@ def kernel_bytes(n, c, nb, cb, g, t):
         "k_boid_density": 20 * nb,
         # S8-S10: read posS 16, velS 16, rho 4, perm 4; write pos' 16, vel' 16
         "k_force_integrate": 72 * n,
+        "k_force_list": 72 * n,     # the stored-neighbour-list variant of the same rows
         # S11-S13: read bpos, bvel 32, rho_b 4, perm 4; write 32
         "k_boid_step": 72 * nb,
         # S14: write phi 4 per corner; read posS 16 per particle and the cell table 8 per cell

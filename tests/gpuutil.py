@@ -20,6 +20,9 @@ def host_u32(t):
     return t.cpu().numpy().view(np.uint32)
 
 
+FORCE_VARIANT = None  # set by a test fixture: 0 = stored neighbour list, 1 = grid walk (sph_set_force_variant)
+
+
 class Sim:
     """One libsphboid context sized for a workload dict (workloads.config)."""
 
@@ -28,6 +31,8 @@ class Sim:
         self.G = G if G is not None else cfg.get("G", 0)
         self.ctx = B.sph_create(cfg["sph"], max_particles or max(cfg["n"], 1), max(cfg.get("n_boid", 0), 1), self.G)
         self.dims, self.C = B.sph_grid_dims(self.ctx)
+        if FORCE_VARIANT is not None:
+            B.sph_set_force_variant(self.ctx, FORCE_VARIANT)
 
     def close(self):
         if self.ctx is not None:

@@ -9,9 +9,18 @@ import pytest
 
 from oracle import refbind as R
 from paper_2311_15088_b200 import workloads as W
+from tests import gpuutil
 from tests.gpuutil import Sim, dev, vec_err
 
 pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(autouse=True, params=[0, 1], ids=["nbrlist", "gridwalk"])
+def force_variant(request):
+    """Every test runs on both S8 kernels: the stored-neighbour-list pass (default) and the grid walk."""
+    gpuutil.FORCE_VARIANT = request.param
+    yield request.param
+    gpuutil.FORCE_VARIANT = None
 
 
 def _compare_step(cfg, out, ref, pos0):
