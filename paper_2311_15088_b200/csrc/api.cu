@@ -29,6 +29,9 @@ struct sph_ctx {
   int force_variant;     // 0 = stored neighbour list (k_force_list), 1 = grid walk (k_force_integrate)
   int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = cell groups, 3 = corner blocks, 4 = corner tiles (mc_set_sdf_variant)
   uint32_t* n_tris_dev;
+  uint2* mc_work;        // [segments] active-segment work list of the surface pass (segment, first triangle)
+  uint32_t* mc_nwork;    // [2] its length, two counters used alternately
+  bool bits_ready;       // mc_bits was filled by the SDF kernel of the mc_extract in progress
   ScanState scan;
   uint32_t max_tiles;
   // sequencing
@@ -255,7 +258,8 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   if (cudaMalloc(&ctx->rhoS, nn * 4) != cudaSuccess || cudaMalloc(&ctx->rho_bS, nb * 4) != cudaSuccess ||
       cudaMalloc(&ctx->phi, std::max<size_t>(G * G * G, 1) * 4) != cudaSuccess ||
       cudaMalloc(&ctx->mc_bits, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4) != cudaSuccess ||
-      cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess || cudaMalloc(&ctx->nbr.cnt, nn * 2) != cudaSuccess ||
+      cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess || cudaMalloc(&ctx->mc_nwork, 8) != cudaSuccess ||
+      cudaMalloc(&ctx->mc_work, std::max<size_t>(mc_num_segments((uint32_t)G), 1) * 8) != cudaSuccess || cudaMalloc(&ctx->nbr.cnt, nn * 2) != cudaSuccess ||
       cudaMalloc(&ctx->nbr.list, (size_t)nbr_rows() * (ctx->nbr.stride = (uint32_t)((nn + 63) & ~(size_t)63)) * 2) != cudaSuccess ||
       cudaMalloc(&ctx->sdf_first, (size_t)(ctx->sdf_first_cap = (uint32_t)(sc.grid.dim[0] + sc.grid.dim[1] +
                                                                           sc.grid.dim[2] + 3 * (2 * 16 + 3))) * 4) !=
@@ -267,6 +271,8 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   cudaMemset(ctx->scan.status, 0, (size_t)ctx->max_tiles * 8);
   cudaMemset(ctx->scan.ticket, 0, 4);
   cudaMemset(ctx->n_tris_dev, 0, 4);
+  cudaMemset(ctx->mc_nwork, 0, 8);
+  cudaMemset(ctx->mc_bits, 0, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4);
   ctx->scan.ticket_base = 0;
   ctx->scan.epoch = 0;
   upload_mc_tables();
@@ -280,7 +286,7 @@ int sph_destroy(sph_ctx* ctx) {
   cudaSetDevice(ctx->device);
   free_grid(ctx->pg);
   free_grid(ctx->bg);
-  cudaFree(ctx->nbr.list), cudaFree(ctx->nbr.cnt), cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->sdf_first);
+  cudaFree(ctx->nbr.list), cudaFree(ctx->nbr.cnt), cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->mc_work), cudaFree(ctx->mc_nwork), cudaFree(ctx->sdf_first);
   cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket);
   sph_profile_enable(ctx, 0);
   free(ctx->prof.recs);
@@ -303,7 +309,7 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step",
-    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_mc_signs", "k_mc_polygonise", "k_zero_u32"};
+    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_zero_u32"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -413,7 +419,7 @@ int boid_step(sph_ctx* ctx, const boid_params* bp, void* bpos, void* bvel, uint3
   return SPH_OK;
 }
 
-int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi) {
+static int voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi, bool want_bits) {
   if (!ctx) return SPH_E_INVALID;
   McConst m;
   int rc = make_mc(ctx, mp, m);
@@ -421,10 +427,15 @@ int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi) {
   if (!phi) return fail(ctx, SPH_E_INVALID, "phi is NULL");
   if (!ctx->grid_fresh) return fail(ctx, SPH_E_STALE_GRID, "mc needs sph_build_grid on the current positions");
   CK(cudaSetDevice(ctx->device));
-  launch_voxel_sdf(ctx->sc, m, ctx->pg, ctx->sdf_first, ctx->sdf_first_cap, phi, ctx->sdf_variant,
-                   (cudaStream_t)stream, &ctx->prof);
+  ctx->bits_ready = launch_voxel_sdf(ctx->sc, m, ctx->pg, ctx->sdf_first, ctx->sdf_first_cap, phi,
+                                     want_bits ? ctx->mc_bits : nullptr, ctx->sdf_variant, (cudaStream_t)stream,
+                                     &ctx->prof);
   CK(cudaGetLastError());
   return SPH_OK;
+}
+
+int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi) {
+  return voxel_sdf(ctx, mp, stream, phi, false);
 }
 
 int mc_set_sdf_variant(sph_ctx* ctx, int variant) {
@@ -441,8 +452,8 @@ int sph_set_force_variant(sph_ctx* ctx, int variant) {
   return SPH_OK;
 }
 
-int mc_polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, void* stream, float* tris,
-                  uint32_t tri_capacity, uint32_t* n_tris_host, uint32_t* n_tris_dev) {
+static int polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, bool bits_ready, void* stream, float* tris,
+                      uint32_t tri_capacity, uint32_t* n_tris_host, uint32_t* n_tris_dev) {
   if (!ctx) return SPH_E_INVALID;
   McConst m;
   int rc = make_mc(ctx, mp, m);
@@ -450,7 +461,8 @@ int mc_polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, void* str
   if (!phi || (tri_capacity > 0 && !tris)) return fail(ctx, SPH_E_INVALID, "phi / tris is NULL");
   cudaStream_t s = (cudaStream_t)stream;
   CK(cudaSetDevice(ctx->device));
-  launch_mc_polygonise(m, phi, ctx->mc_bits, tris, tri_capacity, ctx->n_tris_dev, ctx->scan, s, &ctx->prof);
+  launch_mc_polygonise(m, phi, ctx->mc_bits, bits_ready, tris, tri_capacity, ctx->n_tris_dev, ctx->mc_work,
+                       ctx->mc_nwork, ctx->scan, s, &ctx->prof);
   if (n_tris_dev) CK(cudaMemcpyAsync(n_tris_dev, ctx->n_tris_dev, 4, cudaMemcpyDeviceToDevice, s));
   CK(cudaGetLastError());
   if (n_tris_host) {
@@ -461,13 +473,18 @@ int mc_polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, void* str
   return SPH_OK;
 }
 
+int mc_polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, void* stream, float* tris,
+                  uint32_t tri_capacity, uint32_t* n_tris_host, uint32_t* n_tris_dev) {
+  return polygonise(ctx, mp, phi, false, stream, tris, tri_capacity, n_tris_host, n_tris_dev);
+}
+
 int mc_extract(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi, float* tris, uint32_t tri_capacity,
                uint32_t* n_tris_host) {
   if (!ctx) return SPH_E_INVALID;
   float* field = phi ? phi : ctx->phi;
-  int rc = mc_voxel_sdf(ctx, mp, stream, field);
+  int rc = voxel_sdf(ctx, mp, stream, field, true);
   if (rc != SPH_OK) return rc;
-  return mc_polygonise(ctx, mp, field, stream, tris, tri_capacity, n_tris_host, nullptr);
+  return polygonise(ctx, mp, field, ctx->bits_ready, stream, tris, tri_capacity, n_tris_host, nullptr);
 }
 
 int sph_simulate_host(sph_ctx* ctx, float* pos_host, float* vel_host, uint32_t n, float* bpos_host, float* bvel_host,

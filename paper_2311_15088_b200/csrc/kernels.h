@@ -38,7 +38,7 @@ enum KernelId {
   K_HASH_COUNT = 0, K_SCAN_CELLS, K_SCATTER, K_REORDER,          // particle grid
   K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
   K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
-  K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_MC_SIGNS, K_MC_POLYGONISE, K_ZERO_U32,
+  K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_ZERO_U32,
   K_NUM_KERNELS
 };
 
@@ -109,10 +109,13 @@ void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg,
 // mc.cu
 void upload_mc_tables();
 void mc_table_host(int8_t* tri, uint8_t* ntri);
-void launch_voxel_sdf(const SphConst& c, const McConst& m, const GridBuf& pg, uint32_t* sdf_first,
-                      uint32_t sdf_first_cap, float* phi, int variant, cudaStream_t s, Prof* prof);
-void launch_mc_polygonise(const McConst& m, const float* phi, uint32_t* bits, float* tris, uint32_t capacity,
-                          uint32_t* n_tris_dev, ScanState& scan, cudaStream_t s, Prof* prof);
+bool launch_voxel_sdf(const SphConst& c, const McConst& m, const GridBuf& pg, uint32_t* sdf_first,
+                      uint32_t sdf_first_cap, float* phi, uint32_t* sign_bits /* optional */, int variant,
+                      cudaStream_t s, Prof* prof);  // true if it also filled the corner sign bit field
+void launch_mc_polygonise(const McConst& m, const float* phi, uint32_t* bits, bool bits_ready, float* tris,
+                          uint32_t capacity, uint32_t* n_tris_dev, uint2* work, uint32_t* n_work, ScanState& scan,
+                          cudaStream_t s, Prof* prof);
+uint64_t mc_num_segments(uint32_t G);  // size of the active-segment work list
 uint64_t mc_bits_words(uint32_t G);  // size of the corner sign bit field
 uint32_t mc_num_tiles(uint32_t G);
 

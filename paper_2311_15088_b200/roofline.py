@@ -40,7 +40,8 @@ def kernel_bytes(n, c, nb, cb, g, t):
         "k_sdf_axis_tables": 0,                         # helper of S14 (axis partition tables): bytes counted above
         # S15-S17: read phi 4 per corner, write 36 per triangle
         "k_mc_signs": 4 * v,                            # S15 first half: read phi once -> 1 bit per corner
-        "k_mc_polygonise": 36 * t,                      # S15 second half - S17 on the bit field (G^3 / 8 bytes: < 1 %)
+        "k_mc_count": v // 8,                           # S15 second half - S16 on the bit field (1 bit per corner)
+        "k_mc_emit": 36 * t,                            # S17: 36 B per triangle (+ the few phi values it interpolates)
         "k_zero_u32": 4,
     }
 
@@ -48,7 +49,10 @@ def kernel_bytes(n, c, nb, cb, g, t):
 SIM_KERNELS = ("k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]",
                "k_scan_cells[boid grid]", "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density",
                "k_boid_density", "k_force_integrate", "k_boid_step")
-MC_KERNELS = ("k_voxel_sdf", "k_mc_signs", "k_mc_polygonise")  # one of k_voxel_sdf / k_voxel_sdf_groups runs per pass
+# The surface pass in SURVEY.md 8(d)'s accounting: phi written once and read once (4 + 4 B per corner), particles and
+# cell table read once, 36 B per triangle.  The fused path reads the sign bits instead of phi (k_mc_signs does not run),
+# but the pass figure keeps the survey's 8 B per corner so that it stays comparable.
+MC_KERNELS = ("k_voxel_sdf", "k_mc_signs", "k_mc_emit")
 
 
 def summarise(profile, n, c, nb, cb, g, t, peak_gbs):
