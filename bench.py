@@ -14,7 +14,8 @@ C ABI; torch supplies device memory, streams and events only.  One JSON line is 
              (S14-S17), each with its algorithmic GB/s and fraction of the measured HBM peak
   e2e        the same frame through sph_simulate_host with pinned HOST buffers, copies inside the timed region
   roofline   the dominant kernel: algorithmic bytes per launch / its average CUDA-event duration
-  kernels    every kernel: launches, average us, share of the step, algorithmic GB/s
+  kernels    every kernel: launches, average us, share of the step, algorithmic GB/s (event pairs around every launch,
+             in a second run of the same K frames so that the pairs do not sit inside the region `value` is timed on)
   cpu_baseline  the CPU oracle (oracle/, test infrastructure) timed on this box's host cores on the same workload
 
 --impl reference times the oracle alone (this tier has no reference implementation to install).
@@ -219,7 +220,6 @@ def main():
     time.sleep(0.15)
     ranks.barrier()
     torch.cuda.synchronize()
-    B.sph_profile_enable(fr.ctx, True)
     launches0 = B.sph_launch_count(fr.ctx)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K + 1)]
     ev[0].record()
@@ -234,6 +234,16 @@ def main():
     t_total = ev[0].elapsed_time(ev[2 * K]) * 1e-3
     t_sim = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(K)) * 1e-3
     t_mc = sum(ev[2 * k + 1].elapsed_time(ev[2 * k + 2]) for k in range(K)) * 1e-3
+    # ---- per-kernel durations: the same K frames again with a CUDA event pair around every launch (the pairs cost a
+    # few microseconds per launch, so they stay out of the region `value` is measured on) ----------------------------
+    B.sph_profile_enable(fr.ctx, True)
+    evp = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    evp[0].record()
+    for k in range(K):
+        fr.frame()
+    evp[1].record()
+    torch.cuda.synchronize()
+    t_profiled = evp[0].elapsed_time(evp[1]) * 1e-3
     profile = B.sph_profile_read(fr.ctx)
     B.sph_profile_enable(fr.ctx, False)
     clocks = sampler.stop()
@@ -326,6 +336,9 @@ def main():
             "kernels": [{"kernel": r["kernel"], "launches": r["launches"], "avg_us": round(r["avg_us"], 2),
                          "share": round(r["share"], 4), "gbs": round(r["gbs"], 1), "frac": round(r["frac"], 4)}
                         for r in rows],
+            "kernel_timing": {"how": "the same K frames run a second time with a CUDA event pair around every launch "
+                                     "(on the launching stream); `value` comes from the first, un-instrumented run",
+                              "ms_per_step_instrumented": 1e3 * t_profiled / K},
             "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "cpu_baseline": cpu,
         }
         print(json.dumps(line))
