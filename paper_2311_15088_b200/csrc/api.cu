@@ -44,6 +44,8 @@ struct sph_ctx {
   bool boid_state;       // bg/rho_bS hold the boids given to the last sph_step
   const void* boid_pos;
   uint32_t boid_n;
+  cudaStream_t side;     // the boid grid + probe density of sph_step run here, beside k_density
+  cudaEvent_t ev_fork, ev_join;
   Prof prof;
   char err[256];
   // staging for the *_host entry point
@@ -275,6 +277,10 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   cudaMemset(ctx->mc_bits, 0, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4);
   ctx->scan.ticket_base = 0;
   ctx->scan.epoch = 0;
+  if (cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess)
+    return bail(SPH_E_CUDA);
   upload_mc_tables();
   if (cudaDeviceSynchronize() != cudaSuccess) return bail(SPH_E_CUDA);
   *out = ctx;
@@ -290,6 +296,9 @@ int sph_destroy(sph_ctx* ctx) {
   cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket);
   sph_profile_enable(ctx, 0);
   free(ctx->prof.recs);
+  if (ctx->side) cudaStreamDestroy(ctx->side);
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   cudaFree(ctx->h_pos), cudaFree(ctx->h_vel), cudaFree(ctx->h_bpos), cudaFree(ctx->h_bvel), cudaFree(ctx->h_tris);
   delete ctx;
   return SPH_OK;
@@ -375,15 +384,26 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
   if (!(ctx->grid_fresh && ctx->grid_pos == pos && ctx->grid_vel == vel && ctx->grid_n == n))
     build_grid(ctx, pos, vel, n, s);
   ctx->boid_state = false;
+  const NbrList* nl = ctx->force_variant == 0 ? &ctx->nbr : nullptr;
   if (n_boid > 0) {
     int rc = set_boid_params(ctx, bp);
     if (rc != SPH_OK) return rc;
-    launch_build_grid(ctx->bc.grid, ctx->bg, (const float4*)bpos, (const float4*)bvel, n_boid, ctx->scan, s,
-                      &ctx->prof, true);  // S7 / K14: Boid Space hash, same machinery as the particle grid
+    // S7 / K14 (Boid Space hash, same machinery as the particle grid) and the boids' probe density depend only on the
+    // particle grid, not on rho: they run on the context's side stream beside k_density and join before the forces
+    // (with per-kernel timing on they stay on the caller's stream, so that every event pair brackets one kernel alone)
+    const bool fork = !ctx->prof.on;
+    cudaStream_t sb = fork ? ctx->side : s;
+    if (fork) {
+      CK(cudaEventRecord(ctx->ev_fork, s));
+      CK(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+    }
+    launch_build_grid(ctx->bc.grid, ctx->bg, (const float4*)bpos, (const float4*)bvel, n_boid, ctx->scan, sb, &ctx->prof,
+                      true);
+    launch_boid_density(ctx->sc, ctx->pg, ctx->bg, n_boid, ctx->rho_bS, sb, &ctx->prof);
+    if (fork) CK(cudaEventRecord(ctx->ev_join, ctx->side));
   }
-  const NbrList* nl = ctx->force_variant == 0 ? &ctx->nbr : nullptr;
   launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, nl, s, &ctx->prof);
-  if (n_boid > 0) launch_boid_density(ctx->sc, ctx->pg, ctx->bg, n_boid, ctx->rho_bS, s, &ctx->prof);
+  if (n_boid > 0 && !ctx->prof.on) CK(cudaStreamWaitEvent(s, ctx->ev_join, 0));
   launch_force_integrate(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS,
                          ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, nl, s, &ctx->prof);
   ctx->grid_fresh = false;  // positions moved
