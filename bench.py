@@ -271,10 +271,13 @@ def main():
     mc_gbs = mc_bytes * K / t_mc / 1e9
     dom = next(r for r in rows if r["kernel"] == dominant)
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")  # dram__bytes_read.sum + dram__bytes_write.sum per launch (ncu --set full)
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get(dominant, {}).get("dram_bytes_per_launch")
+            for row in open(tp).read().splitlines()[1:]:
+                c = row.split(",")
+                if c and c[0] == dominant:
+                    traffic = float(c[1])
         except Exception:
             traffic = None
 
