@@ -180,3 +180,10 @@ def test_full_size_mc_config4_sampled():
         nt = B.mc_polygonise(sim.ctx, mp, phi, buf)
         assert nt == nt_ref
         assert np.array_equal(buf.cpu().numpy()[:nt], tris_ref)
+        # the fused path bench.py times (mc_extract: the SDF kernel writes the sign field, no k_mc_signs): same phi
+        # bit for bit, hence the same mesh bit for bit
+        buf2 = torch.zeros(nt_ref + 10, 3, 3, device="cuda")
+        phi2 = torch.zeros(G ** 3, device="cuda")
+        nt2 = B.mc_extract(sim.ctx, mp, buf2, phi=phi2)
+        assert bool((phi2 == phi).all())
+        assert nt2 == nt_ref and np.array_equal(buf2.cpu().numpy()[:nt2], tris_ref)
