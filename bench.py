@@ -13,7 +13,8 @@ C ABI; torch supplies device memory, streams and events only.  One JSON line is 
   parts      the two halves BASELINE.json's metric names: SPH+boid particle-updates/s (S1-S13) and MC voxels/s
              (S14-S17), each with its algorithmic GB/s and fraction of the measured HBM peak
   e2e        the same frame through sph_simulate_host with pinned HOST buffers, copies inside the timed region
-  roofline   the dominant kernel: algorithmic bytes per launch / its average CUDA-event duration
+  roofline   the dominant kernel on the roofline that binds it: binary32 arithmetic (algorithmic flops of the true
+             pairs / its average CUDA-event duration against the FMA peak), with its HBM coordinates under "hbm"
   kernels    every kernel: launches, average us, share of the step, algorithmic GB/s (event pairs around every launch,
              in a second run of the same K frames so that the pairs do not sit inside the region `value` is timed on)
   cpu_baseline  the CPU oracle (oracle/, test infrastructure) timed on this box's host cores on the same workload
@@ -248,6 +249,10 @@ def main():
     B.sph_profile_enable(fr.ctx, False)
     clocks = sampler.stop()
     n_tris = B.mc_extract(fr.ctx, fr.mc, fr.tris, sync=True)  # same state as the last timed frame
+    # true neighbour pairs of that state (for the arithmetic roofline): one more SPH step with the count output
+    ncount = torch.zeros(n, dtype=torch.int32, device=fr.device)
+    B.sph_step(fr.ctx, fr.pos, fr.vel, fr.bpos, fr.bvel, cfg["boid"], ncount=ncount)
+    sph_pairs = float(ncount.sum().item())
     if n_tris > fr.tri_capacity:
         raise SystemExit("triangle buffer too small: %d > %d" % (n_tris, fr.tri_capacity))
     cb = None
@@ -270,6 +275,10 @@ def main():
     sim_gbs = sim_bytes * K / t_sim / 1e9
     mc_gbs = mc_bytes * K / t_mc / 1e9
     dom = next(r for r in rows if r["kernel"] == dominant)
+    sm_max = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("sm_max_mhz", 1965.0)) \
+        if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else 1965.0
+    pairs = RF.sdf_pairs(n, fr.mc["radius"], fr.mc["spacing"]) if RF.KERNEL_KIND.get(dominant) == "sdf" else sph_pairs
+    alu = RF.alu_point(dominant, dom["avg_us"], pairs, sm_max)
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.csv")  # dram__bytes_read.sum + dram__bytes_write.sum per launch (ncu --set full)
     if os.path.exists(tp):
@@ -280,6 +289,19 @@ def main():
                     traffic = float(c[1])
         except Exception:
             traffic = None
+
+    hbm = {"achieved": dom["gbs"], "peak": peak, "unit": "GB/s", "frac": dom["frac"], "peak_kind": "of " + peak_kind,
+           "bytes_per_launch": dom["bytes"]}
+    if alu is not None:
+        # the dominant kernel is bound by binary32 arithmetic (DRAM throughput ~1 % in profiles/): ALU roofline first,
+        # its HBM coordinates (BASELINE.json's metric) beside it
+        roof = {"bound": "alu", "kernel": dominant, "achieved": alu["achieved"], "peak": alu["peak"], "unit": "TFLOP/s",
+                "frac": alu["frac"], "traffic": traffic, "flop_per_launch": alu["flop_per_launch"],
+                "pairs_per_launch": alu["pairs"], "flop_per_pair": alu["flop_per_pair"],
+                "peak_kind": "148 SMs x 128 lanes x 2 flop x %.0f MHz (DESIGN.md section 6)" % sm_max,
+                "avg_us": dom["avg_us"], "share_of_step": dom["share"], "hbm": hbm}
+    else:
+        roof = dict(hbm, bound="hbm", kernel=dominant, traffic=traffic, avg_us=dom["avg_us"], share_of_step=dom["share"])
 
     # ---- end to end through the C ABI with HOST buffers -------------------------------------------------
     e2e = None
@@ -310,7 +332,7 @@ def main():
     # ---- the oracle on this box's host cores, rank 0 at N = 1 only --------------------------------------
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        frames, per, cores = time_oracle(cfg, W.mc_params(cfg), 10.0, 3)
+        frames, per, cores = time_oracle(cfg, W.mc_params(cfg), 10.0, 8)
         cpu = {"value": n * frames / sum(per), "unit": "particle-updates/s", "cores": cores, "kind": "oracle",
                "sample": "%d whole frame(s) of %s (%d particles, %d boids, %d^3 corners), %.1f s" %
                          (frames, cfg["name"], n, nb, G, sum(per))}
@@ -333,9 +355,7 @@ def main():
                 "mc": {"value": G ** 3 * K * world / t_mc_max, "unit": "voxels/s", "ms_per_step": 1e3 * t_mc_max / K,
                        "algorithmic_gbs": mc_gbs, "frac_of_hbm_peak": mc_gbs / peak, "rows": "S14-S17: mc_extract"},
             },
-            "roofline": {"bound": "hbm", "kernel": dominant, "achieved": dom["gbs"], "peak": peak, "unit": "GB/s",
-                         "frac": dom["frac"], "traffic": traffic, "peak_kind": "of " + peak_kind,
-                         "bytes_per_launch": dom["bytes"], "avg_us": dom["avg_us"], "share_of_step": dom["share"]},
+            "roofline": roof,
             "kernels": [{"kernel": r["kernel"], "launches": r["launches"], "avg_us": round(r["avg_us"], 2),
                          "share": round(r["share"], 4), "gbs": round(r["gbs"], 1), "frac": round(r["frac"], 4)}
                         for r in rows],

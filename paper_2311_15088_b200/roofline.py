@@ -76,3 +76,41 @@ def summarise(profile, n, c, nb, cb, g, t, peak_gbs):
 def pass_bytes(names, n, c, nb, cb, g, t):
     kb = kernel_bytes(n, c, nb, cb, g, t)
     return sum(kb[k] for k in names)
+
+
+# ---- arithmetic roofline of the three pair kernels -------------------------------------------
+# The hot kernels are bound by binary32 arithmetic, not by HBM, so bench.py also places the dominant kernel on the
+# ALU roofline: algorithmic flops = (true pairs) x (flops of one pair as the paper's listing evaluates it), peak =
+# 148 SMs x 128 lanes x 2 flop x SM clock (FMA counted as two).  Only true pairs count: candidates that fail the
+# distance test, list building and filters are overhead of the implementation.
+ALU_PEAK_TFLOPS_AT_MHZ = lambda mhz: 148 * 128 * 2 * mhz * 1e6 / 1e12
+
+FLOP_PER_PAIR = {
+    # Listing 9: d = x_j - x (3), r^2 (5), 1 - r^2/R^2 (2), k = u^3 (2), S0 += k (1), S1 += k d (6)
+    "sdf": 19,
+    # Eq. 27: d (3), r^2 (5), h^2 - r^2 (1), cube and accumulate (3)
+    "density": 12,
+    # Listing 3: d, dv (6), r^2 (5), sqrt + q, q2 (4), q2/q (1), pressure factor (4), coefficient (3),
+    # three components of (pterm d - 40 mu dv) scaled and accumulated (12)
+    "force": 35,
+}
+KERNEL_KIND = {"k_voxel_sdf_tiles": "sdf", "k_voxel_sdf_blocks": "sdf", "k_voxel_sdf_groups": "sdf", "k_voxel_sdf": "sdf",
+               "k_density": "density", "k_force_list": "force", "k_force_integrate": "force"}
+
+
+def sdf_pairs(n, radius, spacing):
+    """(corner, particle) pairs with r < R: every particle reaches the corners of a ball of radius R of the voxel
+    lattice, 4/3 pi (R / spacing)^3 of them, when the voxel grid covers the fluid (it does in all five configs)."""
+    import math
+    return n * 4.0 / 3.0 * math.pi * (radius / spacing) ** 3
+
+
+def alu_point(kernel, avg_us, pairs, sm_mhz):
+    kind = KERNEL_KIND.get(kernel)
+    if kind is None or not pairs or avg_us <= 0:
+        return None
+    flops = FLOP_PER_PAIR[kind] * pairs
+    peak = ALU_PEAK_TFLOPS_AT_MHZ(sm_mhz)
+    ach = flops / (avg_us * 1e-6) / 1e12
+    return dict(achieved=ach, peak=peak, frac=ach / peak, flop_per_launch=flops, pairs=pairs,
+                flop_per_pair=FLOP_PER_PAIR[kind])
