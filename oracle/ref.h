@@ -105,6 +105,13 @@ int ref_voxel_sdf(const ref_sph_params* p, const ref_mc_params* mp, const float*
 int ref_mc_polygonise(const ref_mc_params* mp, const float* phi, float* tris, uint32_t tri_capacity,
                       uint32_t* n_tris, uint8_t* case_of_cube);
 
+/* N3 (D:A-NORMAL, D:A-WELD): the same mesh as ref_mc_polygonise, indexed: one vertex per crossing grid edge in
+ * ascending edge key 3*point + axis, verts / normals = vert_capacity*3 floats (normals may be NULL),
+ * indices = tri_capacity*3 vertex ids in ref_mc_polygonise's triangle order.  n_verts / n_tris get the REQUIRED counts;
+ * nothing past a capacity is written.  Returns 1 if a capacity was too small. */
+int ref_mc_indexed(const ref_mc_params* mp, const float* phi, float* verts, float* normals, uint32_t vert_capacity,
+                   uint32_t* indices, uint32_t tri_capacity, uint32_t* n_verts, uint32_t* n_tris);
+
 /* The generated table (D:M-TABLE): tri[256][16] edge ids terminated by -1, ntri[256], edge_table[256]. */
 void ref_mc_table(int8_t* tri, uint8_t* ntri, uint16_t* edge_table);
 /* Bourke numbering used by the table: corner offsets [8][3], edge endpoints [12][2]. */

@@ -6,6 +6,9 @@
 
 #include <math.h>
 #include <string.h>
+
+#include <cmath>
+#include <utility>
 #include <vector>
 
 namespace {
@@ -240,6 +243,100 @@ int ref_mc_polygonise(const ref_mc_params* mp, const float* phi, float* tris, ui
       }
   if (n_tris) *n_tris = (uint32_t)count;
   return count > tri_capacity ? 1 : 0;
+}
+
+// N3: indexed mesh with per-vertex normals.  The paper only says that normals are computed for each
+// vertex and reports connectivity of the triangles; reading D:A-NORMAL / D:A-WELD:
+//  * one vertex per grid edge whose end corners lie on different sides of iso, numbered in ascending edge key
+//    3 * (point index of the edge's lower corner) + axis (x = 0, y = 1, z = 2); its position is Eq. 51 with
+//    p1 = the lower corner (D:A-EDGE), so it is bitwise the vertex ref_mc_polygonise emits for that edge;
+//  * indices[3 t + v] = vertex id of triangle t, corner v, triangles in ref_mc_polygonise's order;
+//  * normal = normalise(g_a + w (g_b - g_a)), g = grad phi at a corner by central differences (one-sided on the
+//    border of the grid), w the weight of Eq. 51; phi grows outwards, so the normal points out of the fluid.
+static void grad_phi(const ref_mc_params* mp, const float* phi, uint32_t i, uint32_t j, uint32_t k, float g[3]) {
+  const uint32_t G = mp->n_point_per_axis;
+  const uint32_t c[3] = {i, j, k};
+  const uint64_t stride[3] = {1, G, (uint64_t)G * G};
+  const uint64_t p = i + (uint64_t)G * (j + (uint64_t)G * k);
+  for (int a = 0; a < 3; ++a) {
+    const bool lo = c[a] > 0, hi = c[a] + 1 < G;
+    const float fm = lo ? phi[p - stride[a]] : phi[p], fp = hi ? phi[p + stride[a]] : phi[p];
+    const float span = (float)((lo ? 1 : 0) + (hi ? 1 : 0)) * mp->spacing;
+    g[a] = span > 0.0f ? (fp - fm) / span : 0.0f;
+  }
+}
+
+int ref_mc_indexed(const ref_mc_params* mp, const float* phi, float* verts, float* normals, uint32_t vert_capacity,
+                   uint32_t* indices, uint32_t tri_capacity, uint32_t* n_verts, uint32_t* n_tris) {
+  const Table& T = table();
+  if (!T.ok) return -2;
+  const uint32_t G = mp->n_point_per_axis;
+  if (n_verts) *n_verts = 0;
+  if (n_tris) *n_tris = 0;
+  if (G < 2) return 0;
+  const float iso = mp->iso;
+  const uint64_t NP = (uint64_t)G * G * G;
+  const uint64_t stride[3] = {1, G, (uint64_t)G * G};
+  std::vector<uint32_t> vid(3 * NP, 0xffffffffu);
+  uint64_t nv = 0;
+  for (uint32_t k = 0; k < G; ++k)
+    for (uint32_t j = 0; j < G; ++j)
+      for (uint32_t i = 0; i < G; ++i) {
+        const uint64_t p = i + (uint64_t)G * (j + (uint64_t)G * k);
+        const uint32_t c[3] = {i, j, k};
+        for (int a = 0; a < 3; ++a) {
+          if (c[a] + 1 >= G) continue;
+          const float va = phi[p], vb = phi[p + stride[a]];
+          if ((va < iso) == (vb < iso)) continue;
+          vid[3 * p + a] = (uint32_t)nv;
+          if (nv < vert_capacity) {
+            const float w = (iso - va) / (vb - va);  // P:546 Eq. 51, p1 = lower corner
+            uint32_t cb[3] = {i, j, k};
+            cb[a] += 1;
+            float ga[3], gb[3], nrm[3];
+            grad_phi(mp, phi, i, j, k, ga);
+            grad_phi(mp, phi, cb[0], cb[1], cb[2], gb);
+            for (int x = 0; x < 3; ++x) {
+              const float pa = mp->origin[x] + (float)c[x] * mp->spacing;
+              const float pb = mp->origin[x] + (float)cb[x] * mp->spacing;
+              if (verts) verts[3 * nv + x] = pa + w * (pb - pa);
+              nrm[x] = ga[x] + w * (gb[x] - ga[x]);
+            }
+            if (normals) {
+              const float len = std::sqrt(nrm[0] * nrm[0] + nrm[1] * nrm[1] + nrm[2] * nrm[2]);
+              for (int x = 0; x < 3; ++x) normals[3 * nv + x] = len > 0.0f ? nrm[x] / len : 0.0f;
+            }
+          }
+          ++nv;
+        }
+      }
+  const uint32_t Q = G - 1;
+  uint64_t count = 0;
+  for (uint32_t k = 0; k < Q; ++k)
+    for (uint32_t j = 0; j < Q; ++j)
+      for (uint32_t i = 0; i < Q; ++i) {
+        uint64_t gidx[8];
+        int cs = 0;
+        for (int n = 0; n < 8; ++n) {
+          gidx[n] = (i + kCorner[n][0]) + (uint64_t)G * ((j + kCorner[n][1]) + (uint64_t)G * (k + kCorner[n][2]));
+          if (phi[gidx[n]] < iso) cs |= 1 << n;
+        }
+        for (int t = 0; T.tri[cs][t] != -1; t += 3) {
+          if (count < tri_capacity && indices)
+            for (int v = 0; v < 3; ++v) {
+              const int e = T.tri[cs][t + v];
+              uint64_t pa = gidx[kEdge[e][0]], pb = gidx[kEdge[e][1]];
+              if (pb < pa) std::swap(pa, pb);
+              const uint64_t d = pb - pa;
+              const int axis = d == 1 ? 0 : (d == G ? 1 : 2);
+              indices[3 * count + v] = vid[3 * pa + axis];
+            }
+          ++count;
+        }
+      }
+  if (n_verts) *n_verts = (uint32_t)nv;
+  if (n_tris) *n_tris = (uint32_t)count;
+  return (nv > vert_capacity || count > tri_capacity) ? 1 : 0;
 }
 
 }  // extern "C"

@@ -58,6 +58,7 @@ def lib():
         L.ref_boid_step.argtypes = [vp, vp, vp, vp, vp, _u32, vp, vp, _u32, C.c_int, vp]
         L.ref_voxel_sdf.argtypes = [vp, vp, vp, _u32, C.c_int, vp]
         L.ref_mc_polygonise.argtypes = [vp, vp, vp, _u32, vp, vp]
+        L.ref_mc_indexed.argtypes = [vp, vp, vp, vp, _u32, vp, _u32, vp, vp]
         L.ref_mc_table.argtypes = [vp, vp, vp]
         L.ref_mc_table.restype = None
         L.ref_mc_numbering.argtypes = [vp, vp]
@@ -184,6 +185,23 @@ def mc_polygonise(mp, phi, capacity=None, want_cases=False):
     rc = lib().ref_mc_polygonise(C.byref(m), _p(phi), _p(tris), capacity, C.byref(nt), _p(cases))
     assert rc in (0, 1)
     return tris[:min(capacity, nt.value)], int(nt.value), cases
+
+
+def mc_indexed(mp, phi):
+    """N3: returns (verts (V,3), normals (V,3), indices (T,3) uint32) of the welded mesh."""
+    m = _fill(McParams, mp)
+    g = int(mp["n_point_per_axis"])
+    phi = np.ascontiguousarray(phi, np.float32)
+    assert phi.size == g ** 3
+    nv, nt = _u32(0), _u32(0)
+    lib().ref_mc_indexed(C.byref(m), _p(phi), None, None, 0, None, 0, C.byref(nv), C.byref(nt))
+    verts = np.zeros((max(nv.value, 1), 3), np.float32)
+    normals = np.zeros((max(nv.value, 1), 3), np.float32)
+    idx = np.zeros((max(nt.value, 1), 3), np.uint32)
+    rc = lib().ref_mc_indexed(C.byref(m), _p(phi), _p(verts), _p(normals), nv.value, _p(idx), nt.value, C.byref(nv),
+                              C.byref(nt))
+    assert rc == 0
+    return verts[:nv.value], normals[:nv.value], idx[:nt.value]
 
 
 def mc_table():

@@ -165,3 +165,74 @@ def test_single_particle_through_sdf_and_mc_gives_sphere_of_radius_rbar():
     v = tris.reshape(-1, 3).astype(np.float64)
     # linear interpolation (Eq. 51) of a distance function along an edge errs by at most spacing^2 / (8 r)
     assert np.abs(np.linalg.norm(v - x1[0, :3], axis=1) - 0.5 * h).max() < 1.1 * mp["spacing"] ** 2 / (8 * 0.5 * h)
+
+
+# ---- N3: indexed mesh with per-vertex normals (D:A-NORMAL, D:A-WELD) ------------------------------------------------
+def _sphere_phi(mp, c, r):
+    x = _corners(mp).astype(np.float64)
+    return (np.linalg.norm(x - np.asarray(c), axis=1) - r).astype(np.float32)
+
+
+def test_indexed_mesh_expands_to_the_triangle_soup_bitwise():
+    # the welded mesh is the same mesh: verts[indices] == ref_mc_polygonise's triangles, bit for bit, on white noise
+    # (all 256 cases) and on a sphere; and welding by bitwise vertex equality (meshutil) finds the same vertex count
+    rng = np.random.default_rng(3)
+    G = 14
+    mp = _mp(G, origin=(0.1, -0.2, 0.3), spacing=0.013, iso=0.1)
+    mp0 = dict(mp, iso=0.0)
+    for mp, phi in ((mp, rng.standard_normal(G ** 3).astype(np.float32)), (mp0, _sphere_phi(mp0, (0.18, -0.12, 0.39), 0.055))):
+        tris, nt, _ = R.mc_polygonise(mp, phi)
+        verts, normals, idx = R.mc_indexed(mp, phi)
+        assert idx.shape[0] == nt and nt > 0
+        assert np.array_equal(verts[idx.astype(np.int64)], tris)
+        # every vertex is used, and its id order is the ascending edge key (x-fastest point order, then axis)
+        assert np.array_equal(np.unique(idx), np.arange(verts.shape[0]))
+    ids, nv = M.weld(tris)  # sphere: no two crossing edges share a position, so bitwise welding agrees
+    assert nv == verts.shape[0]
+
+
+def test_indexed_sphere_is_a_closed_surface_by_index_and_normals_point_outwards():
+    G = 40
+    mp = _mp(G)
+    c, r = (0.5, 0.52, 0.47), 0.3
+    phi = _sphere_phi(mp, c, r)
+    verts, normals, idx = R.mc_indexed(mp, phi)
+    V, F = verts.shape[0], idx.shape[0]
+    E, closed, degenerate = M.edge_stats(idx.astype(np.int64))
+    assert closed and degenerate == 0
+    assert V - E + F == 2  # Euler characteristic of a sphere, now on the index buffer itself
+    # normals: unit length, within 2 degrees of the radial direction (central differences are O(spacing^2) accurate)
+    radial = verts.astype(np.float64) - np.asarray(c)
+    radial /= np.linalg.norm(radial, axis=1, keepdims=True)
+    assert np.abs(np.linalg.norm(normals.astype(np.float64), axis=1) - 1.0).max() < 1e-6
+    assert (np.einsum("ij,ij->i", normals.astype(np.float64), radial)).min() > math.cos(math.radians(2.0))
+    # vertex ids ascend with the edge key 3 * (lower corner) + axis: recover corner and axis from the position (the
+    # coordinate along the edge is the one off the lattice; the other two sit on it)
+    t = (verts.astype(np.float64) - np.float64(mp["origin"])) / float(np.float32(mp["spacing"]))
+    frac = np.abs(t - np.round(t))
+    axis = np.argmax(frac, axis=1)
+    cell = np.round(t).astype(np.int64)
+    rows = np.arange(len(t))
+    cell[rows, axis] = np.floor(t[rows, axis]).astype(np.int64)
+    key = 3 * (cell[:, 0] + G * (cell[:, 1] + G * cell[:, 2])) + axis
+    on_lattice = frac.max(axis=1) < 1e-4  # a vertex that coincides with a corner has no recoverable axis
+    assert on_lattice.mean() < 0.01
+    k = key[~on_lattice]
+    assert np.all(np.diff(k) > 0)
+
+
+def test_indexed_plane_normals_are_exact_and_border_is_one_sided():
+    # phi = z - z0 is linear: central and one-sided differences are exact up to rounding, the normal is (0, 0, 1);
+    # the plane z0 sits in the LAST layer of cubes, so the upper corners use the one-sided border formula
+    G = 9
+    mp = _mp(G, spacing=0.125)
+    z0 = 0.125 * (G - 2) + 0.05
+    x = _corners(mp).astype(np.float64)
+    phi = (x[:, 2] - z0).astype(np.float32)
+    verts, normals, idx = R.mc_indexed(mp, phi)
+    assert verts.shape[0] == G * G and idx.shape[0] == 2 * (G - 1) ** 2
+    assert np.abs(verts[:, 2] - z0).max() < 1e-6
+    assert np.abs(normals - np.array([0, 0, 1], np.float32)).max() < 1e-6
+    # flipped sign: fluid above the plane, normals point down
+    v2, n2, _ = R.mc_indexed(mp, -phi)
+    assert np.array_equal(v2, verts) and np.abs(n2 - np.array([0, 0, -1], np.float32)).max() < 1e-6
