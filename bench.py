@@ -249,6 +249,20 @@ def main():
     B.sph_profile_enable(fr.ctx, False)
     clocks = sampler.stop()
     n_tris = B.mc_extract(fr.ctx, fr.mc, fr.tris, sync=True)  # same state as the last timed frame
+    # N3 (not part of `value`): the same surface as an indexed mesh with normals, timed on its own
+    iverts = torch.empty(3 * max(n_tris, 1), 3, device=fr.device)
+    inorm = torch.empty(3 * max(n_tris, 1), 3, device=fr.device)
+    iidx = torch.empty(max(n_tris, 1), 3, dtype=torch.int32, device=fr.device)
+    n_iv, _ = B.mc_extract_indexed(fr.ctx, fr.mc, iverts, inorm, iidx)
+    evi = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    evi[0].record()
+    for _ in range(3):
+        B.mc_extract_indexed(fr.ctx, fr.mc, iverts, inorm, iidx, sync=False)
+    evi[1].record()
+    torch.cuda.synchronize()
+    indexed = {"ms_per_pass": evi[0].elapsed_time(evi[1]) / 3, "vertices": n_iv, "triangles": n_tris,
+               "what": "mc_extract_indexed: S14 + welded vertices, central-difference normals, index buffer"}
+    del iverts, inorm, iidx
     # true neighbour pairs of that state (for the arithmetic roofline): one more SPH step with the count output
     ncount = torch.zeros(n, dtype=torch.int32, device=fr.device)
     B.sph_step(fr.ctx, fr.pos, fr.vel, fr.bpos, fr.bvel, cfg["boid"], ncount=ncount)
@@ -362,7 +376,7 @@ def main():
             "kernel_timing": {"how": "the same K frames run a second time with a CUDA event pair around every launch "
                                      "(on the launching stream); `value` comes from the first, un-instrumented run",
                               "ms_per_step_instrumented": 1e3 * t_profiled / K},
-            "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "cpu_baseline": cpu,
+            "indexed_mesh": indexed, "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "cpu_baseline": cpu,
         }
         print(json.dumps(line))
     ranks.close()

@@ -135,6 +135,21 @@ int mc_polygonise(sph_ctx* ctx, const mc_params* mp /* host */, const float* phi
 int mc_extract(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, float* phi, float* tris,
                uint32_t tri_capacity, uint32_t* n_tris_host);
 
+/* N3 ("normals ... for each vertex", P:595-602 connectivity; readings D:A-NORMAL, D:A-WELD):
+ * the same surface as mc_polygonise / mc_extract as an INDEXED mesh.  One vertex per grid edge whose end corners lie on
+ * different sides of iso, in ascending edge key 3 * (point index of the lower corner) + axis; verts / normals are
+ * vert_capacity * 3 floats (normals optional: NULL), position = Eq. 51 (bitwise the vertex mc_polygonise emits for that
+ * edge), normal = normalise(g_a + w (g_b - g_a)) with g = grad phi by central differences (one-sided on the grid border).
+ * indices = tri_capacity * 3 vertex ids, triangles in mc_polygonise's order.  *n_verts_host / *n_tris_host (host,
+ * optional; passing either makes the call synchronise) get the REQUIRED counts; SPH_E_CAPACITY if one exceeds its
+ * capacity, nothing past a capacity is written.  All buffers are DEVICE pointers. */
+int mc_polygonise_indexed(sph_ctx* ctx, const mc_params* mp /* host */, const float* phi, void* stream, float* verts,
+                          float* normals, uint32_t vert_capacity, uint32_t* indices, uint32_t tri_capacity,
+                          uint32_t* n_verts_host, uint32_t* n_tris_host);
+int mc_extract_indexed(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, float* phi, float* verts,
+                       float* normals, uint32_t vert_capacity, uint32_t* indices, uint32_t tri_capacity,
+                       uint32_t* n_verts_host, uint32_t* n_tris_host);
+
 /* End-to-end frame with HOST buffers (pinned or pageable): copies pos/vel/bpos/bvel to the device, runs
  * `steps` frames of sph_build_grid + sph_step + boid_step, optionally one surface pass on the final
  * positions (mp != NULL), copies the state (and triangles) back and synchronises.

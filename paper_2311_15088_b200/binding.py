@@ -78,6 +78,8 @@ def lib():
         L.sph_set_force_variant.argtypes = [_vp, C.c_int]
         L.mc_polygonise.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.mc_extract.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp]
+        L.mc_polygonise_indexed.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _u32, _vp, _u32, _vp, _vp]
+        L.mc_extract_indexed.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _u32, _vp, _u32, _vp, _vp]
         L.sph_simulate_host.argtypes = [_vp, _vp, _vp, _u32, _vp, _vp, _u32, _vp, _u32, _vp, _vp, _u32, _vp]
         L.sph_mc_table.argtypes = [_vp, _vp]
         L.sph_mc_table.restype = None
@@ -92,7 +94,7 @@ def lib():
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "mc_polygonise", "mc_extract", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "mc_polygonise", "mc_extract", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
            "sph_profile_read", "sph_kernel_name"]
 
 
@@ -234,6 +236,31 @@ def mc_extract(ctx, mc, tris, phi=None, stream=None, sync=True):
     rc = lib().mc_extract(ctx, C.byref(m), _stream(stream), _ptr(phi), _ptr(tris), cap, C.byref(nt) if sync else None)
     _check(ctx, rc, allow=(SPH_E_CAPACITY,))
     return int(nt.value) if sync else None
+
+
+def mc_polygonise_indexed(ctx, mc, phi, verts, normals, indices, stream=None, sync=True):
+    """N3: indexed mesh of a given phi.  verts / normals (Vcap, 3) float32, indices (Tcap, 3) int32 CUDA tensors
+    (normals may be None).  Returns (n_verts, n_tris) required when sync, else None."""
+    m = _fill(McParams, mc)
+    nv, nt = _u32(0), _u32(0)
+    rc = lib().mc_polygonise_indexed(ctx, C.byref(m), _ptr(phi), _stream(stream), _ptr(verts), _ptr(normals),
+                                     0 if verts is None else verts.shape[0], _ptr(indices),
+                                     0 if indices is None else indices.shape[0], C.byref(nv) if sync else None,
+                                     C.byref(nt) if sync else None)
+    _check(ctx, rc, allow=(SPH_E_CAPACITY,))
+    return (int(nv.value), int(nt.value)) if sync else None
+
+
+def mc_extract_indexed(ctx, mc, verts, normals, indices, phi=None, stream=None, sync=True):
+    """N3: S14 then the indexed mesh (see mc_polygonise_indexed)."""
+    m = _fill(McParams, mc)
+    nv, nt = _u32(0), _u32(0)
+    rc = lib().mc_extract_indexed(ctx, C.byref(m), _stream(stream), _ptr(phi), _ptr(verts), _ptr(normals),
+                                  0 if verts is None else verts.shape[0], _ptr(indices),
+                                  0 if indices is None else indices.shape[0], C.byref(nv) if sync else None,
+                                  C.byref(nt) if sync else None)
+    _check(ctx, rc, allow=(SPH_E_CAPACITY,))
+    return (int(nv.value), int(nt.value)) if sync else None
 
 
 def sph_simulate_host(ctx, pos, vel, bpos=None, bvel=None, boid=None, steps=1, mc=None, tris=None):

@@ -29,6 +29,8 @@ struct sph_ctx {
   int force_variant;     // 0 = stored neighbour list (k_force_list), 1 = grid walk (k_force_integrate)
   int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = cell groups, 3 = corner blocks, 4 = corner tiles (mc_set_sdf_variant)
   uint32_t* n_tris_dev;
+  uint32_t* mc_prefix;   // [words of mc_bits] vertex-id prefix of the indexed mesh (N3)
+  uint32_t* n_verts_dev;
   uint2* mc_work;        // [segments] active-segment work list of the surface pass (segment, first triangle)
   uint32_t* mc_nwork;    // [2] its length, two counters used alternately
   bool bits_ready;       // mc_bits was filled by the SDF kernel of the mc_extract in progress
@@ -260,7 +262,8 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   if (cudaMalloc(&ctx->rhoS, nn * 4) != cudaSuccess || cudaMalloc(&ctx->rho_bS, nb * 4) != cudaSuccess ||
       cudaMalloc(&ctx->phi, std::max<size_t>(G * G * G, 1) * 4) != cudaSuccess ||
       cudaMalloc(&ctx->mc_bits, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4) != cudaSuccess ||
-      cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess || cudaMalloc(&ctx->mc_nwork, 8) != cudaSuccess ||
+      cudaMalloc(&ctx->n_tris_dev, 4) != cudaSuccess || cudaMalloc(&ctx->n_verts_dev, 4) != cudaSuccess ||
+      cudaMalloc(&ctx->mc_prefix, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4) != cudaSuccess || cudaMalloc(&ctx->mc_nwork, 8) != cudaSuccess ||
       cudaMalloc(&ctx->mc_work, std::max<size_t>(mc_num_segments((uint32_t)G), 1) * 8) != cudaSuccess || cudaMalloc(&ctx->nbr.cnt, nn * 2) != cudaSuccess ||
       cudaMalloc(&ctx->nbr.list, (size_t)nbr_rows() * (ctx->nbr.stride = (uint32_t)((nn + 63) & ~(size_t)63)) * 2) != cudaSuccess ||
       cudaMalloc(&ctx->sdf_first, (size_t)(ctx->sdf_first_cap = (uint32_t)(sc.grid.dim[0] + sc.grid.dim[1] +
@@ -268,7 +271,7 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
           cudaSuccess || cudaMalloc(&ctx->scan.ticket, 4) != cudaSuccess)
     return bail(SPH_E_CUDA);
   ctx->max_tiles = std::max(std::max(grid_scan_tiles(sc.grid.C), grid_scan_tiles(ctx->boid_cells_cap)),
-                            std::max(mc_num_tiles((uint32_t)G), 1u));
+                            std::max(std::max(mc_num_tiles((uint32_t)G), mc_word_tiles((uint32_t)G)), 1u));
   if (cudaMalloc(&ctx->scan.status, (size_t)ctx->max_tiles * 8) != cudaSuccess) return bail(SPH_E_CUDA);
   cudaMemset(ctx->scan.status, 0, (size_t)ctx->max_tiles * 8);
   cudaMemset(ctx->scan.ticket, 0, 4);
@@ -292,7 +295,7 @@ int sph_destroy(sph_ctx* ctx) {
   cudaSetDevice(ctx->device);
   free_grid(ctx->pg);
   free_grid(ctx->bg);
-  cudaFree(ctx->nbr.list), cudaFree(ctx->nbr.cnt), cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->mc_work), cudaFree(ctx->mc_nwork), cudaFree(ctx->sdf_first);
+  cudaFree(ctx->nbr.list), cudaFree(ctx->nbr.cnt), cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->n_verts_dev), cudaFree(ctx->mc_prefix), cudaFree(ctx->mc_work), cudaFree(ctx->mc_nwork), cudaFree(ctx->sdf_first);
   cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket);
   sph_profile_enable(ctx, 0);
   free(ctx->prof.recs);
@@ -318,7 +321,7 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step",
-    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_zero_u32"};
+    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -496,6 +499,51 @@ static int polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, bool 
 int mc_polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, void* stream, float* tris,
                   uint32_t tri_capacity, uint32_t* n_tris_host, uint32_t* n_tris_dev) {
   return polygonise(ctx, mp, phi, false, stream, tris, tri_capacity, n_tris_host, n_tris_dev);
+}
+
+static int polygonise_indexed(sph_ctx* ctx, const mc_params* mp, const float* phi, bool bits_ready, void* stream,
+                              float* verts, float* normals, uint32_t vert_capacity, uint32_t* indices,
+                              uint32_t tri_capacity, uint32_t* n_verts_host, uint32_t* n_tris_host) {
+  if (!ctx) return SPH_E_INVALID;
+  McConst m;
+  int rc = make_mc(ctx, mp, m);
+  if (rc != SPH_OK) return rc;
+  if (!phi || (vert_capacity > 0 && !verts) || (tri_capacity > 0 && !indices))
+    return fail(ctx, SPH_E_INVALID, "phi / verts / indices is NULL");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  launch_mc_indexed(m, phi, ctx->mc_bits, bits_ready, ctx->mc_prefix, verts, normals, vert_capacity, indices,
+                    tri_capacity, ctx->n_verts_dev, ctx->n_tris_dev, ctx->mc_work, ctx->mc_nwork, ctx->scan, s,
+                    &ctx->prof);
+  CK(cudaGetLastError());
+  if (n_verts_host || n_tris_host) {
+    uint32_t nv = 0, nt = 0;
+    CK(cudaMemcpyAsync(&nv, ctx->n_verts_dev, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(&nt, ctx->n_tris_dev, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    if (n_verts_host) *n_verts_host = nv;
+    if (n_tris_host) *n_tris_host = nt;
+    if (nv > vert_capacity || nt > tri_capacity) return fail(ctx, SPH_E_CAPACITY, "vertex / index buffer too small");
+  }
+  return SPH_OK;
+}
+
+int mc_polygonise_indexed(sph_ctx* ctx, const mc_params* mp, const float* phi, void* stream, float* verts,
+                          float* normals, uint32_t vert_capacity, uint32_t* indices, uint32_t tri_capacity,
+                          uint32_t* n_verts_host, uint32_t* n_tris_host) {
+  return polygonise_indexed(ctx, mp, phi, false, stream, verts, normals, vert_capacity, indices, tri_capacity,
+                            n_verts_host, n_tris_host);
+}
+
+int mc_extract_indexed(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi, float* verts, float* normals,
+                       uint32_t vert_capacity, uint32_t* indices, uint32_t tri_capacity, uint32_t* n_verts_host,
+                       uint32_t* n_tris_host) {
+  if (!ctx) return SPH_E_INVALID;
+  float* field = phi ? phi : ctx->phi;
+  int rc = voxel_sdf(ctx, mp, stream, field, true);
+  if (rc != SPH_OK) return rc;
+  return polygonise_indexed(ctx, mp, field, ctx->bits_ready, stream, verts, normals, vert_capacity, indices,
+                            tri_capacity, n_verts_host, n_tris_host);
 }
 
 int mc_extract(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi, float* tris, uint32_t tri_capacity,

@@ -38,7 +38,7 @@ enum KernelId {
   K_HASH_COUNT = 0, K_SCAN_CELLS, K_SCATTER, K_REORDER,          // particle grid
   K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
   K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
-  K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_ZERO_U32,
+  K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_MC_EDGE_SCAN, K_MC_VERTICES, K_MC_EMIT_INDICES, K_ZERO_U32,
   K_NUM_KERNELS
 };
 
@@ -115,6 +115,11 @@ bool launch_voxel_sdf(const SphConst& c, const McConst& m, const GridBuf& pg, ui
 void launch_mc_polygonise(const McConst& m, const float* phi, uint32_t* bits, bool bits_ready, float* tris,
                           uint32_t capacity, uint32_t* n_tris_dev, uint2* work, uint32_t* n_work, ScanState& scan,
                           cudaStream_t s, Prof* prof);
+void launch_mc_indexed(const McConst& m, const float* phi, uint32_t* bits, bool bits_ready, uint32_t* prefix,
+                       float* verts, float* normals, uint32_t vert_capacity, uint32_t* indices, uint32_t tri_capacity,
+                       uint32_t* n_verts_dev, uint32_t* n_tris_dev, uint2* work, uint32_t* n_work, ScanState& scan,
+                       cudaStream_t s, Prof* prof);
+uint32_t mc_word_tiles(uint32_t G);    // look-back tiles of the edge scan
 uint64_t mc_num_segments(uint32_t G);  // size of the active-segment work list
 uint64_t mc_bits_words(uint32_t G);  // size of the corner sign bit field
 uint32_t mc_num_tiles(uint32_t G);

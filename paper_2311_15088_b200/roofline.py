@@ -42,6 +42,10 @@ def kernel_bytes(n, c, nb, cb, g, t):
         "k_mc_signs": 4 * v,                            # S15 first half: read phi once -> 1 bit per corner
         "k_mc_count": v // 8,                           # S15 second half - S16 on the bit field (1 bit per corner)
         "k_mc_emit": 36 * t,                            # S17: 36 B per triangle (+ the few phi values it interpolates)
+        # N3 (indexed mesh): bit field once more, 24 B per vertex (position + normal), 12 B per triangle
+        "k_mc_edge_scan": v // 8 + v // 8,
+        "k_mc_vertices": 0,
+        "k_mc_emit_indices": 12 * t,
         "k_zero_u32": 4,
     }
 

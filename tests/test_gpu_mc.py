@@ -187,3 +187,74 @@ def test_full_size_mc_config4_sampled():
         nt2 = B.mc_extract(sim.ctx, mp, buf2, phi=phi2)
         assert bool((phi2 == phi).all())
         assert nt2 == nt_ref and np.array_equal(buf2.cpu().numpy()[:nt2], tris_ref)
+
+
+# ---- N3: indexed mesh with per-vertex normals ------------------------------------------------------------------------
+def _indexed_gpu(sim, mp, phi_np, vcap, tcap, with_normals=True):
+    verts = torch.zeros(max(vcap, 1), 3, device="cuda")
+    normals = torch.zeros(max(vcap, 1), 3, device="cuda") if with_normals else None
+    idx = torch.zeros(max(tcap, 1), 3, dtype=torch.int32, device="cuda")
+    nv, nt = B.mc_polygonise_indexed(sim.ctx, mp, dev(phi_np), verts, normals, idx)
+    return (verts.cpu().numpy(), normals.cpu().numpy() if with_normals else None,
+            idx.cpu().numpy().view(np.uint32), nv, nt)
+
+
+@pytest.mark.parametrize("G,kind", [(23, "noise"), (33, "noise"), (40, "sphere"), (70, "sphere")])
+def test_indexed_mesh_matches_oracle_stage_isolated(G, kind):
+    # integers (vertex count, triangle count, every index) and vertex positions bit-exact; normals to 1e-5
+    rng = np.random.default_rng(G)
+    mp = dict(origin=(0.1, -0.2, 0.3), spacing=0.013, n_point_per_axis=G, radius=0.05, particle_radius=0.02,
+              iso=0.1 if kind == "noise" else 0.0)
+    if kind == "noise":
+        phi = rng.standard_normal(G ** 3).astype(np.float32)
+    else:
+        k, j, i = np.meshgrid(np.arange(G), np.arange(G), np.arange(G), indexing="ij")
+        x = np.stack([i, j, k], -1).reshape(-1, 3) * 0.013 + np.array(mp["origin"])
+        c = np.array(mp["origin"]) + 0.013 * (G - 1) * np.array([0.5, 0.47, 0.52])
+        phi = (np.linalg.norm(x - c, axis=1) - 0.013 * (G - 1) * 0.31).astype(np.float32)
+    v_ref, n_ref, i_ref = R.mc_indexed(mp, phi)
+    with Sim(dict(sph=W.config(1)["sph"], n=1), G=G) as sim:
+        v, nrm, idx, nv, nt = _indexed_gpu(sim, mp, phi, v_ref.shape[0] + 5, i_ref.shape[0] + 5)
+        assert nv == v_ref.shape[0] and nt == i_ref.shape[0] and nv > 0
+        assert np.array_equal(idx[:nt], i_ref)
+        assert np.array_equal(v[:nv], v_ref)
+        assert np.abs(nrm[:nv] - n_ref).max() <= 1e-5
+        # without normals, and with capacities that are too small: required counts reported, nothing past capacity
+        v2, _, idx2, nv2, nt2 = _indexed_gpu(sim, mp, phi, nv, nt, with_normals=False)
+        assert nv2 == nv and nt2 == nt and np.array_equal(v2[:nv], v_ref) and np.array_equal(idx2[:nt], i_ref)
+        vcap, tcap = nv // 3, nt // 2
+        verts = torch.full((vcap + 20, 3), -7.0, device="cuda")
+        ind = torch.full((tcap + 20, 3), -7, dtype=torch.int32, device="cuda")
+        import ctypes as C
+        m = B._fill(B.McParams, mp)
+        gv, gt = C.c_uint32(0), C.c_uint32(0)
+        rc = B.lib().mc_polygonise_indexed(sim.ctx, C.byref(m), C.c_void_p(dev(phi).data_ptr()), None,
+                                           C.c_void_p(verts.data_ptr()), None, vcap, C.c_void_p(ind.data_ptr()), tcap,
+                                           C.byref(gv), C.byref(gt))
+        assert rc == B.SPH_E_CAPACITY and gv.value == nv and gt.value == nt
+        assert np.array_equal(verts.cpu().numpy()[:vcap], v_ref[:vcap]) and bool((verts[vcap:] == -7.0).all())
+        assert np.array_equal(ind.cpu().numpy().view(np.uint32)[:tcap], i_ref[:tcap]) and bool((ind[tcap:] == -7).all())
+
+
+def test_indexed_extract_on_config_matches_triangle_soup():
+    # end to end on a fluid config: the indexed mesh expands to exactly the triangles mc_extract emits (same phi)
+    cfg = W.config(2)
+    mp = W.mc_params(cfg)
+    G = mp["n_point_per_axis"]
+    with Sim(cfg, G=G) as sim:
+        B.sph_build_grid(sim.ctx, dev(cfg["pos"]))
+        buf = torch.zeros(400000, 3, 3, device="cuda")
+        phi = torch.zeros(G ** 3, device="cuda")
+        nt = B.mc_extract(sim.ctx, mp, buf, phi=phi)
+        verts = torch.zeros(3 * nt + 8, 3, device="cuda")
+        normals = torch.zeros(3 * nt + 8, 3, device="cuda")
+        idx = torch.zeros(nt + 8, 3, dtype=torch.int32, device="cuda")
+        nv, nt2 = B.mc_extract_indexed(sim.ctx, mp, verts, normals, idx)
+        assert nt2 == nt and 0 < nv < 3 * nt
+        tri = verts.cpu().numpy()[idx.cpu().numpy()[:nt].astype(np.int64)]
+        assert np.array_equal(tri, buf.cpu().numpy()[:nt])
+        v_ref, n_ref, i_ref = R.mc_indexed(mp, phi.cpu().numpy())
+        assert nv == v_ref.shape[0] and np.array_equal(idx.cpu().numpy().view(np.uint32)[:nt], i_ref)
+        assert np.abs(normals.cpu().numpy()[:nv] - n_ref).max() <= 1e-5
+        ln = np.linalg.norm(normals.cpu().numpy()[:nv].astype(np.float64), axis=1)
+        assert np.abs(ln[ln > 0] - 1.0).max() < 1e-5
