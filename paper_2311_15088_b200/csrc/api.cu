@@ -592,6 +592,16 @@ int sph_simulate_host(sph_ctx* ctx, float* pos_host, float* vel_host, uint32_t n
     rc = boid_step(ctx, bp, ctx->h_bpos, ctx->h_bvel, n_boid, s, nullptr);
     if (rc != SPH_OK) return rc;
   }
+  // the final state goes back to the host on the side stream while the surface pass runs (pinned host buffers
+  // make the two overlap; pageable ones are still correct)
+  CK(cudaEventRecord(ctx->ev_fork, s));
+  CK(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+  CK(cudaMemcpyAsync(pos_host, ctx->h_pos, (size_t)n * 16, cudaMemcpyDeviceToHost, ctx->side));
+  CK(cudaMemcpyAsync(vel_host, ctx->h_vel, (size_t)n * 16, cudaMemcpyDeviceToHost, ctx->side));
+  if (n_boid) {
+    CK(cudaMemcpyAsync(bpos_host, ctx->h_bpos, (size_t)n_boid * 16, cudaMemcpyDeviceToHost, ctx->side));
+    CK(cudaMemcpyAsync(bvel_host, ctx->h_bvel, (size_t)n_boid * 16, cudaMemcpyDeviceToHost, ctx->side));
+  }
   int result = SPH_OK;
   uint32_t nt = 0;
   if (mp) {
@@ -604,12 +614,7 @@ int sph_simulate_host(sph_ctx* ctx, float* pos_host, float* vel_host, uint32_t n
     if (got && tris_host) CK(cudaMemcpyAsync(tris_host, ctx->h_tris, (size_t)got * 36, cudaMemcpyDeviceToHost, s));
   }
   if (n_tris_host) *n_tris_host = nt;
-  CK(cudaMemcpyAsync(pos_host, ctx->h_pos, (size_t)n * 16, cudaMemcpyDeviceToHost, s));
-  CK(cudaMemcpyAsync(vel_host, ctx->h_vel, (size_t)n * 16, cudaMemcpyDeviceToHost, s));
-  if (n_boid) {
-    CK(cudaMemcpyAsync(bpos_host, ctx->h_bpos, (size_t)n_boid * 16, cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync(bvel_host, ctx->h_bvel, (size_t)n_boid * 16, cudaMemcpyDeviceToHost, s));
-  }
+  CK(cudaStreamSynchronize(ctx->side));
   CK(cudaStreamSynchronize(s));
   return result;
 }

@@ -1,0 +1,50 @@
+"""The end-to-end entry point with HOST buffers (sph_simulate_host, what bench.py's `e2e` times) against the oracle."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import refbind as R
+from paper_2311_15088_b200 import binding as B
+from paper_2311_15088_b200 import workloads as W
+from tests.gpuutil import Sim, vec_err
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("pinned", [True, False])
+def test_simulate_host_one_frame_matches_oracle(pinned):
+    cfg = W.config(1)
+    mp = W.mc_params(cfg)
+    G, h = mp["n_point_per_axis"], cfg["sph"]["h"]
+    ref = R.step(cfg["sph"], cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"], cfg["boid"])
+    refb = R.boid_step(cfg["sph"], cfg["boid"], cfg["pos"], cfg["vel"], ref["density"], cfg["bpos"], cfg["bvel"])
+    phi_ref = R.voxel_sdf(cfg["sph"], mp, ref["pos"])
+    _, nt_ref, _ = R.mc_polygonise(mp, phi_ref)
+
+    def host(a):
+        t = torch.from_numpy(np.ascontiguousarray(a).copy())
+        return t.pin_memory() if pinned else t
+
+    pos, vel, bpos, bvel = host(cfg["pos"]), host(cfg["vel"]), host(cfg["bpos"]), host(cfg["bvel"])
+    tris = torch.zeros(nt_ref + 64, 3, 3)
+    if pinned:
+        tris = tris.pin_memory()
+    with Sim(cfg, G=G) as sim:
+        nt = B.sph_simulate_host(sim.ctx, pos, vel, bpos, bvel, cfg["boid"], 1, mp, tris)
+        for got, want, what in ((pos, ref["pos"], "pos"), (vel, ref["vel"], "vel"), (bpos, refb["bpos"], "bpos"),
+                                (bvel, refb["bvel"], "bvel")):
+            bad, worst = vec_err(got.numpy()[:, :3], want[:, :3])
+            assert bad == 0, (what, bad, worst)
+        # the mesh is that of the GPU's own phi on the new positions: same count as the device path, and as the oracle's
+        # unless a corner sits within the phi tolerance of iso
+        risky = int((np.abs(phi_ref - mp["iso"]) <= 1e-5 * h).sum())
+        assert abs(nt - nt_ref) <= 5 * 8 * risky and nt > 0
+        buf = torch.zeros(nt + 64, 3, 3, device="cuda")
+        B.sph_build_grid(sim.ctx, pos.cuda())
+        assert B.mc_extract(sim.ctx, mp, buf) == nt
+        assert np.array_equal(buf.cpu().numpy()[:nt], tris.numpy()[:nt])
+        # capacity too small: the required count still comes back
+        small = torch.zeros(max(nt // 4, 1), 3, 3)
+        pos2, vel2 = host(cfg["pos"]), host(cfg["vel"])
+        nt2 = B.sph_simulate_host(sim.ctx, pos2, vel2, host(cfg["bpos"]), host(cfg["bvel"]), cfg["boid"], 1, mp, small)
+        assert nt2 == nt and np.array_equal(pos2.numpy(), pos.numpy())
