@@ -44,10 +44,11 @@ struct sph_ctx {
   bool step_state;       // pg/rhoS hold the step-start state of the last sph_step
   BoidConst bc;
   bool boid_state;       // bg/rho_bS hold the boids given to the last sph_step
+  bool rho_event;        // ev_rho was recorded by that sph_step (boid_step may then use the side stream)
   const void* boid_pos;
   uint32_t boid_n;
   cudaStream_t side;     // the boid grid + probe density of sph_step run here, beside k_density
-  cudaEvent_t ev_fork, ev_join;
+  cudaEvent_t ev_fork, ev_join, ev_rho;  // ev_rho: k_density of the last sph_step has finished
   Prof prof;
   char err[256];
   // staging for the *_host entry point
@@ -282,7 +283,8 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   ctx->scan.epoch = 0;
   if (cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess)
+      cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_rho, cudaEventDisableTiming) != cudaSuccess)
     return bail(SPH_E_CUDA);
   upload_mc_tables();
   if (cudaDeviceSynchronize() != cudaSuccess) return bail(SPH_E_CUDA);
@@ -302,6 +304,7 @@ int sph_destroy(sph_ctx* ctx) {
   if (ctx->side) cudaStreamDestroy(ctx->side);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+  if (ctx->ev_rho) cudaEventDestroy(ctx->ev_rho);
   cudaFree(ctx->h_pos), cudaFree(ctx->h_vel), cudaFree(ctx->h_bpos), cudaFree(ctx->h_bvel), cudaFree(ctx->h_tris);
   delete ctx;
   return SPH_OK;
@@ -406,7 +409,11 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     if (fork) CK(cudaEventRecord(ctx->ev_join, ctx->side));
   }
   launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, nl, s, &ctx->prof);
-  if (n_boid > 0 && !ctx->prof.on) CK(cudaStreamWaitEvent(s, ctx->ev_join, 0));
+  ctx->rho_event = n_boid > 0 && !ctx->prof.on;
+  if (ctx->rho_event) {
+    CK(cudaEventRecord(ctx->ev_rho, s));
+    CK(cudaStreamWaitEvent(s, ctx->ev_join, 0));
+  }
   launch_force_integrate(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS,
                          ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, nl, s, &ctx->prof);
   ctx->grid_fresh = false;  // positions moved
@@ -435,8 +442,20 @@ int boid_step(sph_ctx* ctx, const boid_params* bp, void* bpos, void* bvel, uint3
   if (rc != SPH_OK) return rc;
   if (memcmp(&keep, &ctx->bc.grid, sizeof(GridDesc)) != 0)
     return fail(ctx, SPH_E_STALE_GRID, "boid ranges / space changed since sph_step");
-  launch_boid_step(ctx->sc, ctx->bc, ctx->pg, ctx->bg, ctx->grid_n, n_boid, ctx->rhoS, ctx->rho_bS, (float4*)bpos,
-                   (float4*)bvel, (float4*)dv_parts, s, &ctx->prof);
+  // S11-S13 need the step-start sorted state, rho and rho_b, not the forces: the kernel goes to the side stream, behind
+  // the boid grid / probe density it already ran there and behind k_density (ev_rho), so it runs beside k_force_list;
+  // the caller's stream then waits for it, so everything enqueued after this call still sees the new boid state
+  // (with per-kernel timing on it stays on the caller's stream)
+  if (!ctx->prof.on && ctx->rho_event) {
+    CK(cudaStreamWaitEvent(ctx->side, ctx->ev_rho, 0));
+    launch_boid_step(ctx->sc, ctx->bc, ctx->pg, ctx->bg, ctx->grid_n, n_boid, ctx->rhoS, ctx->rho_bS, (float4*)bpos,
+                     (float4*)bvel, (float4*)dv_parts, ctx->side, &ctx->prof);
+    CK(cudaEventRecord(ctx->ev_join, ctx->side));
+    CK(cudaStreamWaitEvent(s, ctx->ev_join, 0));
+  } else {
+    launch_boid_step(ctx->sc, ctx->bc, ctx->pg, ctx->bg, ctx->grid_n, n_boid, ctx->rhoS, ctx->rho_bS, (float4*)bpos,
+                     (float4*)bvel, (float4*)dv_parts, s, &ctx->prof);
+  }
   ctx->boid_state = false;  // boids moved
   CK(cudaGetLastError());
   return SPH_OK;
