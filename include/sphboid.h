@@ -135,6 +135,18 @@ int mc_polygonise(sph_ctx* ctx, const mc_params* mp /* host */, const float* phi
 int mc_extract(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, float* phi, float* tris,
                uint32_t tri_capacity, uint32_t* n_tris_host);
 
+/* The surface pass of frame t and the SPH step of frame t+1 are independent once the grid on the new positions exists
+ * (the mesh is only rendered), and they stress different units (FMA pipe vs L1 / load latency).
+ * mc_extract_async enqueues S14-S17 on a stream of the context, ordered after everything already enqueued on `stream`,
+ * and returns without making `stream` wait; sph_step / boid_step enqueued afterwards on `stream` run beside it.  The
+ * library itself orders the next sph_build_grid (which overwrites what the pass reads) and any other mc_* call after
+ * the pending pass.  phi / tris must stay untouched until mc_wait, which makes `stream` wait for the pass and, if
+ * n_tris_host (host) is given, synchronises and returns the required count (SPH_E_CAPACITY as for mc_extract).
+ * One pass can be pending at a time; results are those of mc_extract, bit for bit. */
+int mc_extract_async(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, float* phi, float* tris,
+                     uint32_t tri_capacity);
+int mc_wait(sph_ctx* ctx, void* stream, uint32_t* n_tris_host);
+
 /* N3 ("normals ... for each vertex", P:595-602 connectivity; readings D:A-NORMAL, D:A-WELD):
  * the same surface as mc_polygonise / mc_extract as an INDEXED mesh.  One vertex per grid edge whose end corners lie on
  * different sides of iso, in ascending edge key 3 * (point index of the lower corner) + axis; verts / normals are

@@ -78,6 +78,8 @@ def lib():
         L.sph_set_force_variant.argtypes = [_vp, C.c_int]
         L.mc_polygonise.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.mc_extract.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp]
+        L.mc_extract_async.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32]
+        L.mc_wait.argtypes = [_vp, _vp, _vp]
         L.mc_polygonise_indexed.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _u32, _vp, _u32, _vp, _vp]
         L.mc_extract_indexed.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _u32, _vp, _u32, _vp, _vp]
         L.sph_simulate_host.argtypes = [_vp, _vp, _vp, _u32, _vp, _vp, _u32, _vp, _u32, _vp, _vp, _u32, _vp]
@@ -94,7 +96,7 @@ def lib():
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "mc_polygonise", "mc_extract", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
            "sph_profile_read", "sph_kernel_name"]
 
 
@@ -234,6 +236,21 @@ def mc_extract(ctx, mc, tris, phi=None, stream=None, sync=True):
     nt = _u32(0)
     cap = 0 if tris is None else tris.shape[0]
     rc = lib().mc_extract(ctx, C.byref(m), _stream(stream), _ptr(phi), _ptr(tris), cap, C.byref(nt) if sync else None)
+    _check(ctx, rc, allow=(SPH_E_CAPACITY,))
+    return int(nt.value) if sync else None
+
+
+def mc_extract_async(ctx, mc, tris, phi=None, stream=None):
+    """S14-S17 on the context's surface stream, beside whatever is enqueued on `stream` afterwards; see mc_wait."""
+    m = _fill(McParams, mc)
+    cap = 0 if tris is None else tris.shape[0]
+    return _check(ctx, lib().mc_extract_async(ctx, C.byref(m), _stream(stream), _ptr(phi), _ptr(tris), cap))
+
+
+def mc_wait(ctx, stream=None, sync=True):
+    """Orders `stream` after the pending surface pass; returns the required triangle count when sync."""
+    nt = _u32(0)
+    rc = lib().mc_wait(ctx, _stream(stream), C.byref(nt) if sync else None)
     _check(ctx, rc, allow=(SPH_E_CAPACITY,))
     return int(nt.value) if sync else None
 

@@ -48,6 +48,11 @@ struct sph_ctx {
   const void* boid_pos;
   uint32_t boid_n;
   cudaStream_t side;     // the boid grid + probe density of sph_step run here, beside k_density
+  cudaStream_t surf;     // mc_extract_async runs the surface pass here, beside the next frame's SPH step
+  cudaEvent_t ev_surf_fork, ev_surf_done;
+  bool surf_pending;     // a surface pass was forked and nothing has waited for it yet
+  uint32_t surf_capacity;
+  ScanState scan_mc;     // look-back state of the surface pass (its scans may run beside the grid scans)
   cudaEvent_t ev_fork, ev_join, ev_rho;  // ev_rho: k_density of the last sph_step has finished
   Prof prof;
   char err[256];
@@ -213,6 +218,8 @@ int make_mc(sph_ctx* ctx, const mc_params* mp, McConst& m) {
 }
 
 int build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, cudaStream_t s) {
+  // a surface pass forked by mc_extract_async still reads the sorted arrays and the cell table this overwrites
+  if (ctx->surf_pending) cudaStreamWaitEvent(s, ctx->ev_surf_done, 0);
   launch_build_grid(ctx->sc.grid, ctx->pg, (const float4*)pos, (const float4*)vel, n, ctx->scan, s, &ctx->prof, false);
   ctx->grid_pos = pos;
   ctx->grid_vel = vel;
@@ -276,12 +283,24 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   if (cudaMalloc(&ctx->scan.status, (size_t)ctx->max_tiles * 8) != cudaSuccess) return bail(SPH_E_CUDA);
   cudaMemset(ctx->scan.status, 0, (size_t)ctx->max_tiles * 8);
   cudaMemset(ctx->scan.ticket, 0, 4);
+  {
+    const size_t mt = std::max(std::max(mc_num_tiles((uint32_t)G), mc_word_tiles((uint32_t)G)), 1u);
+    if (cudaMalloc(&ctx->scan_mc.status, mt * 8) != cudaSuccess || cudaMalloc(&ctx->scan_mc.ticket, 4) != cudaSuccess)
+      return bail(SPH_E_CUDA);
+    cudaMemset(ctx->scan_mc.status, 0, mt * 8);
+    cudaMemset(ctx->scan_mc.ticket, 0, 4);
+    ctx->scan_mc.ticket_base = 0;
+    ctx->scan_mc.epoch = 0;
+  }
   cudaMemset(ctx->n_tris_dev, 0, 4);
   cudaMemset(ctx->mc_nwork, 0, 8);
   cudaMemset(ctx->mc_bits, 0, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4);
   ctx->scan.ticket_base = 0;
   ctx->scan.epoch = 0;
   if (cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&ctx->surf, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_surf_fork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_surf_done, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_rho, cudaEventDisableTiming) != cudaSuccess)
@@ -298,10 +317,13 @@ int sph_destroy(sph_ctx* ctx) {
   free_grid(ctx->pg);
   free_grid(ctx->bg);
   cudaFree(ctx->nbr.list), cudaFree(ctx->nbr.cnt), cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->n_verts_dev), cudaFree(ctx->mc_prefix), cudaFree(ctx->mc_work), cudaFree(ctx->mc_nwork), cudaFree(ctx->sdf_first);
-  cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket);
+  cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket), cudaFree(ctx->scan_mc.status), cudaFree(ctx->scan_mc.ticket);
   sph_profile_enable(ctx, 0);
   free(ctx->prof.recs);
   if (ctx->side) cudaStreamDestroy(ctx->side);
+  if (ctx->surf) cudaStreamDestroy(ctx->surf);
+  if (ctx->ev_surf_fork) cudaEventDestroy(ctx->ev_surf_fork);
+  if (ctx->ev_surf_done) cudaEventDestroy(ctx->ev_surf_done);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->ev_rho) cudaEventDestroy(ctx->ev_rho);
@@ -463,6 +485,7 @@ int boid_step(sph_ctx* ctx, const boid_params* bp, void* bpos, void* bvel, uint3
 
 static int voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi, bool want_bits) {
   if (!ctx) return SPH_E_INVALID;
+  if (ctx->surf_pending) cudaStreamWaitEvent((cudaStream_t)stream, ctx->ev_surf_done, 0);  // shared phi / sign field
   McConst m;
   int rc = make_mc(ctx, mp, m);
   if (rc != SPH_OK) return rc;
@@ -497,6 +520,7 @@ int sph_set_force_variant(sph_ctx* ctx, int variant) {
 static int polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, bool bits_ready, void* stream, float* tris,
                       uint32_t tri_capacity, uint32_t* n_tris_host, uint32_t* n_tris_dev) {
   if (!ctx) return SPH_E_INVALID;
+  if (ctx->surf_pending) cudaStreamWaitEvent((cudaStream_t)stream, ctx->ev_surf_done, 0);
   McConst m;
   int rc = make_mc(ctx, mp, m);
   if (rc != SPH_OK) return rc;
@@ -504,7 +528,7 @@ static int polygonise(sph_ctx* ctx, const mc_params* mp, const float* phi, bool 
   cudaStream_t s = (cudaStream_t)stream;
   CK(cudaSetDevice(ctx->device));
   launch_mc_polygonise(m, phi, ctx->mc_bits, bits_ready, tris, tri_capacity, ctx->n_tris_dev, ctx->mc_work,
-                       ctx->mc_nwork, ctx->scan, s, &ctx->prof);
+                       ctx->mc_nwork, ctx->scan_mc, s, &ctx->prof);
   if (n_tris_dev) CK(cudaMemcpyAsync(n_tris_dev, ctx->n_tris_dev, 4, cudaMemcpyDeviceToDevice, s));
   CK(cudaGetLastError());
   if (n_tris_host) {
@@ -524,6 +548,7 @@ static int polygonise_indexed(sph_ctx* ctx, const mc_params* mp, const float* ph
                               float* verts, float* normals, uint32_t vert_capacity, uint32_t* indices,
                               uint32_t tri_capacity, uint32_t* n_verts_host, uint32_t* n_tris_host) {
   if (!ctx) return SPH_E_INVALID;
+  if (ctx->surf_pending) cudaStreamWaitEvent((cudaStream_t)stream, ctx->ev_surf_done, 0);
   McConst m;
   int rc = make_mc(ctx, mp, m);
   if (rc != SPH_OK) return rc;
@@ -532,7 +557,7 @@ static int polygonise_indexed(sph_ctx* ctx, const mc_params* mp, const float* ph
   cudaStream_t s = (cudaStream_t)stream;
   CK(cudaSetDevice(ctx->device));
   launch_mc_indexed(m, phi, ctx->mc_bits, bits_ready, ctx->mc_prefix, verts, normals, vert_capacity, indices,
-                    tri_capacity, ctx->n_verts_dev, ctx->n_tris_dev, ctx->mc_work, ctx->mc_nwork, ctx->scan, s,
+                    tri_capacity, ctx->n_verts_dev, ctx->n_tris_dev, ctx->mc_work, ctx->mc_nwork, ctx->scan_mc, s,
                     &ctx->prof);
   CK(cudaGetLastError());
   if (n_verts_host || n_tris_host) {
@@ -572,6 +597,41 @@ int mc_extract(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi, floa
   int rc = voxel_sdf(ctx, mp, stream, field, true);
   if (rc != SPH_OK) return rc;
   return polygonise(ctx, mp, field, ctx->bits_ready, stream, tris, tri_capacity, n_tris_host, nullptr);
+}
+
+int mc_extract_async(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi, float* tris, uint32_t tri_capacity) {
+  if (!ctx) return SPH_E_INVALID;
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  if (ctx->prof.on) {  // per-kernel timing: everything stays on the caller's stream
+    int rc = mc_extract(ctx, mp, stream, phi, tris, tri_capacity, nullptr);
+    if (rc != SPH_OK) return rc;
+    CK(cudaEventRecord(ctx->ev_surf_done, s));
+  } else {
+    CK(cudaEventRecord(ctx->ev_surf_fork, s));
+    CK(cudaStreamWaitEvent(ctx->surf, ctx->ev_surf_fork, 0));
+    int rc = mc_extract(ctx, mp, ctx->surf, phi, tris, tri_capacity, nullptr);
+    if (rc != SPH_OK) return rc;
+    CK(cudaEventRecord(ctx->ev_surf_done, ctx->surf));
+  }
+  ctx->surf_pending = true;
+  ctx->surf_capacity = tri_capacity;
+  return SPH_OK;
+}
+
+int mc_wait(sph_ctx* ctx, void* stream, uint32_t* n_tris_host) {
+  if (!ctx) return SPH_E_INVALID;
+  if (!ctx->surf_pending) return fail(ctx, SPH_E_INVALID, "mc_wait without a pending mc_extract_async");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  CK(cudaStreamWaitEvent(s, ctx->ev_surf_done, 0));
+  ctx->surf_pending = false;
+  if (n_tris_host) {
+    CK(cudaMemcpyAsync(n_tris_host, ctx->n_tris_dev, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    if (*n_tris_host > ctx->surf_capacity) return fail(ctx, SPH_E_CAPACITY, "triangle buffer too small");
+  }
+  return SPH_OK;
 }
 
 int sph_simulate_host(sph_ctx* ctx, float* pos_host, float* vel_host, uint32_t n, float* bpos_host, float* bvel_host,

@@ -60,6 +60,16 @@ class Frame:
             self.n_tris = nt
         return nt
 
+    def surface_async(self):
+        """S14-S17 of this frame beside the next frame's SPH step (mc_extract_async); pair with wait()."""
+        B.mc_extract_async(self.ctx, self.mc, self.tris)
+
+    def wait(self, sync=False):
+        nt = B.mc_wait(self.ctx, sync=sync)
+        if sync:
+            self.n_tris = nt
+        return nt
+
     def frame(self, sync=False):
         self.sim()
         if self.with_mc:

@@ -48,3 +48,36 @@ def test_simulate_host_one_frame_matches_oracle(pinned):
         pos2, vel2 = host(cfg["pos"]), host(cfg["vel"])
         nt2 = B.sph_simulate_host(sim.ctx, pos2, vel2, host(cfg["bpos"]), host(cfg["bvel"]), cfg["boid"], 1, mp, small)
         assert nt2 == nt and np.array_equal(pos2.numpy(), pos.numpy())
+
+
+def test_async_surface_pass_is_bitwise_the_synchronous_one():
+    # three frames: (a) sph_step, boid_step, build_grid, mc_extract in stream order; (b) the same with the surface pass
+    # forked by mc_extract_async and running beside the NEXT frame's SPH step.  State and meshes must be identical bit
+    # for bit, frame by frame (the library orders the next grid build after the pending pass)
+    from paper_2311_15088_b200.pipeline import Frame
+    cfg = W.config(2, scale=2)
+    meshes = []
+    with Frame(cfg) as fa:
+        for _ in range(3):
+            fa.sim()
+            nt = fa.surface(sync=True)
+            meshes.append((nt, fa.tris[:nt].cpu().numpy().copy(), fa.pos.cpu().numpy().copy()))
+    with Frame(cfg) as fb:
+        bufs = [torch.zeros_like(fb.tris) for _ in range(3)]
+        counts, states = [], []
+        for t in range(3):
+            fb.sim()
+            if t > 0:
+                counts.append(fb.wait(sync=True))  # frame t-1's mesh: its pass overlapped this frame's sph_step
+            fb.tris = bufs[t]
+            fb.surface_async()
+            states.append(fb.pos.clone())
+        counts.append(fb.wait(sync=True))
+        torch.cuda.synchronize()
+        for t in range(3):
+            nt, tris, pos = meshes[t]
+            assert counts[t] == nt and nt > 0
+            assert np.array_equal(bufs[t][:nt].cpu().numpy(), tris)
+            assert np.array_equal(states[t].cpu().numpy(), pos)
+        with pytest.raises(B.SphError):
+            B.mc_wait(fb.ctx)  # nothing pending any more
