@@ -96,6 +96,19 @@ int ref_boid_step(const ref_sph_params* p, const ref_boid_params* bp,
                   const float* pos, const float* vel, const float* density, uint32_t n,
                   float* bpos, float* bvel, uint32_t n_boid, int brute, float* dv_parts);
 
+/* N4 (P:261 Obstacle Grid, P:336 step 7; reading D:C-OBST): obstacle avoidance, applied to the boids'
+ * state AFTER the position update (step 7 follows step 6).  The Obstacle Grid is dims[0]*dims[1]*dims[2] cells of size
+ * `cell` from `origin`; normals[4*c] holds the averaged mesh normal of cell c = cx + dims0*(cy + dims1*cz) (zero =
+ * no obstacle there), x_c its centre.  bvel_b += w_obs * sum over cells with |bpos_b - x_c| < visible of g * n_c,
+ * g = heavy if |bpos_b - x_c| < protect else 1.  brute != 0 visits every cell instead of the cells in range. */
+typedef struct {
+  float origin[3], cell;
+  uint32_t dims[3];
+  float w_obs, heavy;
+} ref_obstacle_params;
+int ref_boid_obstacles(const ref_obstacle_params* op, const float* normals, float protect_range, float visible_range,
+                       const float* bpos, float* bvel, uint32_t n_boid, int brute);
+
 /* S14: phi[G^3], corner index i + G*(j + G*k). */
 int ref_voxel_sdf(const ref_sph_params* p, const ref_mc_params* mp, const float* pos, uint32_t n,
                   int brute, float* phi);

@@ -6,6 +6,8 @@
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
+#include <algorithm>
+#include <cmath>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -476,6 +478,46 @@ void ref_pair_term(float mass, float radius, float stiffness, float rest_density
   out[0] = t[0];
   out[1] = t[1];
   out[2] = t[2];
+}
+
+// N4: obstacle avoidance (P:261, P:336 step 7; D:C-OBST).  Sums in binary64, rounded once, like the other boid rules.
+int ref_boid_obstacles(const ref_obstacle_params* op, const float* normals, float protect_range, float visible_range,
+                       const float* bpos, float* bvel, uint32_t n_boid, int brute) {
+  if (!op || !normals || !(op->cell > 0.0f)) return -1;
+  const int dx = (int)op->dims[0], dy = (int)op->dims[1], dz = (int)op->dims[2];
+  const float vis2 = visible_range * visible_range, prot2 = protect_range * protect_range;
+#pragma omp parallel for schedule(static)
+  for (int64_t b = 0; b < (int64_t)n_boid; ++b) {
+    const float* p = bpos + 4 * b;
+    int lo[3] = {0, 0, 0}, hi[3] = {dx - 1, dy - 1, dz - 1};
+    if (!brute) {
+      const int dims[3] = {dx, dy, dz};
+      for (int a = 0; a < 3; ++a) {  // cells whose centre can lie within the visible range
+        const int c0 = (int)std::floor((p[a] - visible_range - op->origin[a]) / op->cell) - 1;
+        const int c1 = (int)std::floor((p[a] + visible_range - op->origin[a]) / op->cell) + 1;
+        lo[a] = std::max(c0, 0);
+        hi[a] = std::min(c1, dims[a] - 1);
+      }
+    }
+    double acc[3] = {0.0, 0.0, 0.0};
+    for (int cz = lo[2]; cz <= hi[2]; ++cz)
+      for (int cy = lo[1]; cy <= hi[1]; ++cy)
+        for (int cx = lo[0]; cx <= hi[0]; ++cx) {
+          const float* nc = normals + 4 * ((size_t)cx + (size_t)dx * ((size_t)cy + (size_t)dy * (size_t)cz));
+          if (nc[0] == 0.0f && nc[1] == 0.0f && nc[2] == 0.0f) continue;
+          const float ex = p[0] - (op->origin[0] + ((float)cx + 0.5f) * op->cell);
+          const float ey = p[1] - (op->origin[1] + ((float)cy + 0.5f) * op->cell);
+          const float ez = p[2] - (op->origin[2] + ((float)cz + 0.5f) * op->cell);
+          const float d2 = std::fmaf(ez, ez, std::fmaf(ey, ey, ex * ex));
+          if (!(d2 < vis2)) continue;
+          const float g = d2 < prot2 ? op->heavy : 1.0f;
+          acc[0] += (double)(g * nc[0]);
+          acc[1] += (double)(g * nc[1]);
+          acc[2] += (double)(g * nc[2]);
+        }
+    for (int a = 0; a < 3; ++a) bvel[4 * b + a] = (float)((double)bvel[4 * b + a] + (double)op->w_obs * acc[a]);
+  }
+  return 0;
 }
 
 }  // extern "C"

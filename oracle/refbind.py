@@ -23,6 +23,10 @@ class BoidParams(C.Structure):
                 ("w_push", _f), ("space_min", _f * 3), ("space_max", _f * 3)]
 
 
+class ObstacleParams(C.Structure):
+    _fields_ = [("origin", _f * 3), ("cell", _f), ("dims", _u32 * 3), ("w_obs", _f), ("heavy", _f)]
+
+
 class McParams(C.Structure):
     _fields_ = [("origin", _f * 3), ("spacing", _f), ("n_point_per_axis", _u32), ("radius", _f),
                 ("particle_radius", _f), ("iso", _f)]
@@ -35,7 +39,8 @@ def _fill(struct, d):
             continue
         v = d[name]
         if hasattr(ctype, "_length_"):
-            setattr(s, name, ctype(*[float(x) for x in v]))
+            conv = int if ctype._type_ is C.c_uint32 else float
+            setattr(s, name, ctype(*[conv(x) for x in v]))
         else:
             setattr(s, name, v)
     return s
@@ -56,6 +61,7 @@ def lib():
         L.ref_boid_density.argtypes = [vp, vp, _u32, vp, _u32, C.c_int, vp]
         L.ref_step.argtypes = [vp, vp, vp, _u32, vp, vp, _u32, vp, C.c_int, vp, vp, vp, vp, vp]
         L.ref_boid_step.argtypes = [vp, vp, vp, vp, vp, _u32, vp, vp, _u32, C.c_int, vp]
+        L.ref_boid_obstacles.argtypes = [vp, vp, _f, _f, vp, vp, _u32, C.c_int]
         L.ref_voxel_sdf.argtypes = [vp, vp, vp, _u32, C.c_int, vp]
         L.ref_mc_polygonise.argtypes = [vp, vp, vp, _u32, vp, vp]
         L.ref_mc_indexed.argtypes = [vp, vp, vp, vp, _u32, vp, _u32, vp, vp]
@@ -158,6 +164,18 @@ def boid_step(sp, bp, pos, vel, rho, bpos, bvel, brute=False):
                              nb, int(brute), _p(parts))
     assert rc == 0
     return dict(bpos=bpos, bvel=bvel, dv_parts=parts)
+
+
+def boid_obstacles(op, normals, protect_range, visible_range, bpos, bvel, brute=False):
+    """N4: obstacle avoidance on the post-update boid state.  normals (cells, 4) float32.  Returns the new bvel."""
+    o = _fill(ObstacleParams, op)
+    normals = np.ascontiguousarray(normals, np.float32)
+    assert normals.shape == (int(np.prod(op["dims"])), 4)
+    bpos, bvel = _f4(bpos), _f4(bvel).copy()
+    rc = lib().ref_boid_obstacles(C.byref(o), _p(normals), protect_range, visible_range, _p(bpos), _p(bvel),
+                                  bpos.shape[0], int(brute))
+    assert rc == 0
+    return bvel
 
 
 def voxel_sdf(sp, mp, pos, brute=False):

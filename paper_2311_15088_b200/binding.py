@@ -46,7 +46,8 @@ def _fill(struct, d):
             continue
         v = d[name]
         if hasattr(ctype, "_length_"):
-            setattr(s, name, ctype(*[float(x) for x in v]))
+            conv = int if ctype._type_ is C.c_uint32 else float
+            setattr(s, name, ctype(*[conv(x) for x in v]))
         else:
             setattr(s, name, v)
     return s

@@ -142,3 +142,25 @@ def mc_params(cfg, pos=None):
 def random_cloud(n, lo, hi, seed):
     """Uniform random points (tests: brute-force pins)."""
     return uniform_box(n, lo, hi, seed, 40)
+
+
+def sphere_obstacle(space_min, space_max, cell, centre, radius, w_obs=0.05, heavy=2.0):
+    """Synthetic Obstacle Grid (stands in for the paper's obstacle meshes): a grid of `cell`
+    over the Boid Space whose cells within half a cell diagonal of the sphere's surface carry the outward unit normal of
+    the sphere at the cell centre, all others zero.  Returns (obstacle params dict, normals (cells, 4) float32).
+    Input construction only: the avoidance rule itself lives in oracle/ and csrc/."""
+    lo = np.asarray(space_min, np.float64)
+    hi = np.asarray(space_max, np.float64)
+    dims = np.maximum(1, np.ceil((hi - lo) / cell)).astype(np.int64)
+    cz, cy, cx = np.meshgrid(np.arange(dims[2]), np.arange(dims[1]), np.arange(dims[0]), indexing="ij")
+    xc = np.stack([np.float32(lo[0]) + (cx.astype(np.float32) + np.float32(0.5)) * np.float32(cell),
+                   np.float32(lo[1]) + (cy.astype(np.float32) + np.float32(0.5)) * np.float32(cell),
+                   np.float32(lo[2]) + (cz.astype(np.float32) + np.float32(0.5)) * np.float32(cell)], -1).reshape(-1, 3)
+    d = xc.astype(np.float64) - np.asarray(centre, np.float64)
+    r = np.linalg.norm(d, axis=1)
+    on = np.abs(r - radius) <= 0.5 * np.sqrt(3.0) * cell
+    normals = np.zeros((xc.shape[0], 4), np.float32)
+    normals[on, :3] = (d[on] / r[on, None]).astype(np.float32)
+    op = dict(origin=tuple(float(np.float32(v)) for v in lo), cell=float(np.float32(cell)),
+              dims=tuple(int(v) for v in dims), w_obs=float(w_obs), heavy=float(heavy))
+    return op, normals

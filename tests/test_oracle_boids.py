@@ -112,3 +112,64 @@ def test_one_particle_one_boid_antisymmetry():
     r = np.linalg.norm(pos[0, :3].astype(np.float64) - bpos[0, :3].astype(np.float64))
     rho_b = R.boid_density(sp, pos, bpos)
     assert np.allclose(rho_b[0], m * (R.w_poly6(0, h) + R.w_poly6(r, h)), rtol=1e-6)
+
+
+# ---- N4: obstacle avoidance (P:261, P:336 step 7; reading D:C-OBST: parity unpinned beyond these invariants) --------
+def _one_cell_grid(normal, cell=0.1, dims=(5, 5, 5), which=(2, 2, 2), w_obs=0.25, heavy=3.0):
+    op = dict(origin=(0.0, 0.0, 0.0), cell=cell, dims=dims, w_obs=w_obs, heavy=heavy)
+    normals = np.zeros((int(np.prod(dims)), 4), np.float32)
+    normals[which[0] + dims[0] * (which[1] + dims[1] * which[2]), :3] = normal
+    centre = (np.array(which) + 0.5) * cell
+    return op, normals, centre
+
+
+def test_obstacle_single_cell_hand_values():
+    # one cell with normal n at centre x_c: inside the protection range the boid gets w * heavy * n, between the protection
+    # and the visual range w * n, beyond the visual range nothing; the position is untouched (step 7 follows step 6)
+    n = np.array([0.6, -0.8, 0.0], np.float32)
+    op, normals, xc = _one_cell_grid(n)
+    protect, visible = 0.05, 0.12
+    bpos = np.zeros((4, 4), np.float32)
+    bpos[0, :3] = xc + [0.03, 0.0, 0.0]    # inside protect
+    bpos[1, :3] = xc + [0.0, 0.08, 0.0]    # between protect and visible
+    bpos[2, :3] = xc + [0.0, 0.0, 0.13]    # outside visible
+    bpos[3, :3] = xc + [0.12, 0.0, 0.0]    # exactly at the visible range: strict '<', nothing
+    bvel = np.tile(np.array([0.1, 0.2, 0.3, 7.0], np.float32), (4, 1))
+    out = R.boid_obstacles(op, normals, protect, visible, bpos, bvel)
+    w, hv = np.float32(0.25), np.float32(3.0)
+    assert np.allclose(out[0, :3], bvel[0, :3] + w * hv * n, atol=1e-7)
+    assert np.allclose(out[1, :3], bvel[1, :3] + w * n, atol=1e-7)
+    assert np.array_equal(out[2], bvel[2]) and np.array_equal(out[3], bvel[3])
+    assert np.array_equal(out[:, 3], bvel[:, 3])  # payload lane carried through
+
+
+def test_obstacle_zero_grid_is_identity_and_range_walk_equals_all_cells():
+    from paper_2311_15088_b200 import workloads as W
+    rng = np.random.default_rng(4)
+    bpos = np.zeros((300, 4), np.float32)
+    bpos[:, :3] = rng.uniform(-0.1, 1.1, (300, 3))  # some boids outside the grid
+    bvel = rng.uniform(-0.2, 0.2, (300, 4)).astype(np.float32)
+    op, normals = W.sphere_obstacle((0, 0, 0), (1, 1, 1), 0.05, (0.5, 0.45, 0.55), 0.25)
+    assert np.array_equal(R.boid_obstacles(op, np.zeros_like(normals), 0.05, 0.1, bpos, bvel), bvel)
+    a = R.boid_obstacles(op, normals, 0.06, 0.13, bpos, bvel)
+    b = R.boid_obstacles(op, normals, 0.06, 0.13, bpos, bvel, brute=True)
+    assert np.array_equal(a, b) and (a != bvel).any()
+
+
+def test_obstacle_sphere_pushes_boids_outwards():
+    # a boid near a spherical obstacle is pushed along the outward normal: the radial component of its velocity grows,
+    # more for the one inside the protection range of the surface cells
+    from paper_2311_15088_b200 import workloads as W
+    c, r = np.array([0.5, 0.5, 0.5]), 0.2
+    op, normals = W.sphere_obstacle((0, 0, 0), (1, 1, 1), 0.04, c, r, w_obs=0.1, heavy=2.0)
+    dirs = np.array([[1, 0, 0], [0, -1, 0], [0.6, 0.0, 0.8]], np.float64)
+    bpos = np.zeros((6, 4), np.float32)
+    bpos[:3, :3] = c + dirs * (r + 0.01)   # hugging the surface
+    bpos[3:, :3] = c + dirs * (r + 0.09)   # further out, still in visual range
+    bvel = np.zeros((6, 4), np.float32)
+    out = R.boid_obstacles(op, normals, 0.05, 0.12, bpos, bvel)
+    radial = np.einsum("ij,ij->i", out[:, :3].astype(np.float64), np.vstack([dirs, dirs]))
+    assert (radial > 0).all() and (radial[:3] > radial[3:]).all()
+    far = np.zeros((1, 4), np.float32)
+    far[0, :3] = c + [0.45, 0, 0]
+    assert np.array_equal(R.boid_obstacles(op, normals, 0.05, 0.12, far, np.zeros((1, 4), np.float32)), np.zeros((1, 4), np.float32))
