@@ -107,6 +107,19 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
 int boid_step(sph_ctx* ctx, const boid_params* bp /* host */, void* bpos, void* bvel, uint32_t n_boid,
               void* stream, void* dv_parts);
 
+/* N4 (P:261 Obstacle Grid, P:336 step 7 "Obstacle Avoidance"; reading D:C-OBST).  An Obstacle Grid of
+ * dims[0]*dims[1]*dims[2] cells of size `cell` from `origin`; normals = DEVICE float4[cells], cell
+ * c = cx + dims0*(cy + dims1*cz) holds the averaged mesh normal of the obstacle surface in that cell (zero = none),
+ * caller-owned and read by every later boid_step until cleared (op or normals NULL).  After its position update each
+ * boid gets v_b += w_obs * sum over the cells whose centre lies within visible_range of the boid of g * n_c, g = heavy
+ * inside protect_range ("weighed heavier"), else 1. */
+typedef struct {
+  float origin[3], cell;
+  uint32_t dims[3];
+  float w_obs, heavy;
+} obstacle_params;
+int boid_set_obstacles(sph_ctx* ctx, const obstacle_params* op /* host */, const void* normals);
+
 /* S8 has two kernels that compute the same forces: 0 (default) = the density pass stores each
  * particle's neighbour list (the paper's section 9 design) and the force pass reads it; 1 = the force pass
  * walks the 27 cells again.  Tests and A/B measurements force one. */

@@ -26,6 +26,10 @@ class BoidParams(C.Structure):
                 ("w_push", _f), ("space_min", _f * 3), ("space_max", _f * 3)]
 
 
+class ObstacleParams(C.Structure):
+    _fields_ = [("origin", _f * 3), ("cell", _f), ("dims", _u32 * 3), ("w_obs", _f), ("heavy", _f)]
+
+
 class McParams(C.Structure):
     _fields_ = [("origin", _f * 3), ("spacing", _f), ("n_point_per_axis", _u32), ("radius", _f),
                 ("particle_radius", _f), ("iso", _f)]
@@ -76,6 +80,7 @@ def lib():
         L.boid_step.argtypes = [_vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.mc_voxel_sdf.argtypes = [_vp, _vp, _vp, _vp]
         L.mc_set_sdf_variant.argtypes = [_vp, C.c_int]
+        L.boid_set_obstacles.argtypes = [_vp, _vp, _vp]
         L.sph_set_force_variant.argtypes = [_vp, C.c_int]
         L.mc_polygonise.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.mc_extract.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp]
@@ -97,7 +102,7 @@ def lib():
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "boid_set_obstacles", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
            "sph_profile_read", "sph_kernel_name"]
 
 
@@ -211,6 +216,14 @@ def boid_step(ctx, boid, bpos, bvel, stream=None, dv_parts=None):
 def mc_voxel_sdf(ctx, mc, phi, stream=None):
     m = _fill(McParams, mc)
     return _check(ctx, lib().mc_voxel_sdf(ctx, C.byref(m), _stream(stream), _ptr(phi)))
+
+
+def boid_set_obstacles(ctx, op, normals):
+    """N4: Obstacle Grid for the boids (op dict + (cells, 4) float32 CUDA tensor that must stay alive), or None to clear."""
+    if op is None or normals is None:
+        return _check(ctx, lib().boid_set_obstacles(ctx, None, None))
+    o = _fill(ObstacleParams, op)
+    return _check(ctx, lib().boid_set_obstacles(ctx, C.byref(o), _ptr(normals)))
 
 
 def sph_set_force_variant(ctx, variant):

@@ -43,6 +43,8 @@ struct sph_ctx {
   bool grid_fresh;       // pg holds a grid of (grid_pos, grid_n) and positions have not moved since
   bool step_state;       // pg/rhoS hold the step-start state of the last sph_step
   BoidConst bc;
+  ObstacleConst oc;      // N4: Obstacle Grid set by boid_set_obstacles (normals stay caller-owned)
+  const float4* obst_normals;
   bool boid_state;       // bg/rho_bS hold the boids given to the last sph_step
   bool rho_event;        // ev_rho was recorded by that sph_step (boid_step may then use the side stream)
   const void* boid_pos;
@@ -345,7 +347,7 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
-    "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step",
+    "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step", "k_boid_obstacles",
     "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
@@ -472,11 +474,17 @@ int boid_step(sph_ctx* ctx, const boid_params* bp, void* bpos, void* bvel, uint3
     CK(cudaStreamWaitEvent(ctx->side, ctx->ev_rho, 0));
     launch_boid_step(ctx->sc, ctx->bc, ctx->pg, ctx->bg, ctx->grid_n, n_boid, ctx->rhoS, ctx->rho_bS, (float4*)bpos,
                      (float4*)bvel, (float4*)dv_parts, ctx->side, &ctx->prof);
+    if (ctx->obst_normals)  // step 7 follows the position update
+      launch_boid_obstacles(ctx->oc, ctx->obst_normals, ctx->bc, (const float4*)bpos, (float4*)bvel, n_boid, ctx->side,
+                            &ctx->prof);
     CK(cudaEventRecord(ctx->ev_join, ctx->side));
     CK(cudaStreamWaitEvent(s, ctx->ev_join, 0));
   } else {
     launch_boid_step(ctx->sc, ctx->bc, ctx->pg, ctx->bg, ctx->grid_n, n_boid, ctx->rhoS, ctx->rho_bS, (float4*)bpos,
                      (float4*)bvel, (float4*)dv_parts, s, &ctx->prof);
+    if (ctx->obst_normals)
+      launch_boid_obstacles(ctx->oc, ctx->obst_normals, ctx->bc, (const float4*)bpos, (float4*)bvel, n_boid, s,
+                            &ctx->prof);
   }
   ctx->boid_state = false;  // boids moved
   CK(cudaGetLastError());
@@ -501,6 +509,23 @@ static int voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi
 
 int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi) {
   return voxel_sdf(ctx, mp, stream, phi, false);
+}
+
+int boid_set_obstacles(sph_ctx* ctx, const obstacle_params* op, const void* normals) {
+  if (!ctx) return SPH_E_INVALID;
+  if (!op || !normals) {  // clear
+    ctx->obst_normals = nullptr;
+    return SPH_OK;
+  }
+  if (!(op->cell > 0.0f) || op->dims[0] == 0 || op->dims[1] == 0 || op->dims[2] == 0 || !aligned16(normals) ||
+      (uint64_t)op->dims[0] * op->dims[1] * op->dims[2] > (1ull << 31))
+    return fail(ctx, SPH_E_INVALID, "bad obstacle grid");
+  for (int a = 0; a < 3; ++a) ctx->oc.origin[a] = op->origin[a], ctx->oc.dims[a] = (int)op->dims[a];
+  ctx->oc.cell = op->cell;
+  ctx->oc.w_obs = op->w_obs;
+  ctx->oc.heavy = op->heavy;
+  ctx->obst_normals = (const float4*)normals;
+  return SPH_OK;
 }
 
 int mc_set_sdf_variant(sph_ctx* ctx, int variant) {

@@ -134,6 +134,51 @@ k_boid_step(SphConst c, BoidConst bc, const float4* __restrict__ posS, const flo
   }
 }
 
+// N4 (P:261 Obstacle Grid, P:336 step 7; D:C-OBST): obstacle avoidance on the boids' state after the
+// position update.  v_b += w_obs * sum over the Obstacle Grid cells whose centre x_c lies within the visual range of
+// g * n_c, g = heavy inside the protection range.  One warp per boid, lanes stride over the cells of the range.
+__global__ void __launch_bounds__(kThreads)
+k_boid_obstacles(ObstacleConst oc, const float4* __restrict__ normals, float prot2, float vis2, float visible,
+                 const float4* __restrict__ bpos, float4* __restrict__ bvel, uint32_t nb) {
+  const uint32_t b = (blockIdx.x * kThreads + threadIdx.x) >> 5;
+  const uint32_t lane = threadIdx.x & 31u;
+  if (b >= nb) return;
+  const float4 p = __ldg(bpos + b);
+  const float pc[3] = {p.x, p.y, p.z};
+  int lo[3], n[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {  // cells whose centre can lie within the visual range (one cell of slack each side)
+    const int c0 = __float2int_rd(__fdiv_rn(pc[a] - visible - oc.origin[a], oc.cell)) - 1;
+    const int c1 = __float2int_rd(__fdiv_rn(pc[a] + visible - oc.origin[a], oc.cell)) + 1;
+    lo[a] = max(c0, 0);
+    n[a] = max(min(c1, oc.dims[a] - 1) - lo[a] + 1, 0);
+  }
+  const uint32_t total = (uint32_t)n[0] * (uint32_t)n[1] * (uint32_t)n[2];
+  double acc[3] = {0.0, 0.0, 0.0};
+  for (uint32_t t = lane; t < total; t += 32) {
+    const uint32_t tz = t / ((uint32_t)n[0] * (uint32_t)n[1]), r = t - tz * (uint32_t)n[0] * (uint32_t)n[1];
+    const uint32_t ty = r / (uint32_t)n[0], tx = r - ty * (uint32_t)n[0];
+    const int cx = lo[0] + (int)tx, cy = lo[1] + (int)ty, cz = lo[2] + (int)tz;
+    const float4 nc = __ldg(normals + (size_t)cx + (size_t)oc.dims[0] * ((size_t)cy + (size_t)oc.dims[1] * (size_t)cz));
+    if (nc.x == 0.0f && nc.y == 0.0f && nc.z == 0.0f) continue;
+    const float ex = __fsub_rn(p.x, __fadd_rn(oc.origin[0], __fmul_rn((float)cx + 0.5f, oc.cell)));
+    const float ey = __fsub_rn(p.y, __fadd_rn(oc.origin[1], __fmul_rn((float)cy + 0.5f, oc.cell)));
+    const float ez = __fsub_rn(p.z, __fadd_rn(oc.origin[2], __fmul_rn((float)cz + 0.5f, oc.cell)));
+    const float d2 = dist2(ex, ey, ez);
+    if (!(d2 < vis2)) continue;
+    const float g = d2 < prot2 ? oc.heavy : 1.0f;
+    acc[0] += (double)__fmul_rn(g, nc.x);
+    acc[1] += (double)__fmul_rn(g, nc.y);
+    acc[2] += (double)__fmul_rn(g, nc.z);
+  }
+#pragma unroll
+  for (int a = 0; a < 3; ++a) acc[a] = warp_sum_f64(acc[a]);
+  if (lane != 0) return;
+  const float4 v = bvel[b];
+  bvel[b] = make_float4((float)((double)v.x + (double)oc.w_obs * acc[0]), (float)((double)v.y + (double)oc.w_obs * acc[1]),
+                        (float)((double)v.z + (double)oc.w_obs * acc[2]), v.w);
+}
+
 }  // namespace
 
 void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
@@ -145,6 +190,16 @@ void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg,
   prof->begin(K_BOID_STEP, s);
   k_boid_step<<<(nb + warps_per_block - 1) / warps_per_block, kThreads, 0, s>>>(
       c, bc, pg.posS, pg.velS, rhoS, pg.start, bg.posS, bg.velS, rho_bS, bg.start, bg.perm, nb, bpos, bvel, dv_parts);
+  prof->end(s);
+}
+
+void launch_boid_obstacles(const ObstacleConst& oc, const float4* normals, const BoidConst& bc, const float4* bpos,
+                           float4* bvel, uint32_t nb, cudaStream_t s, Prof* prof) {
+  if (nb == 0) return;
+  const uint32_t warps_per_block = kThreads / 32;
+  prof->begin(K_BOID_OBSTACLES, s);
+  k_boid_obstacles<<<(nb + warps_per_block - 1) / warps_per_block, kThreads, 0, s>>>(oc, normals, bc.prot2, bc.vis2,
+                                                                                     bc.visible, bpos, bvel, nb);
   prof->end(s);
 }
 

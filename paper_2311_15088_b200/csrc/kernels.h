@@ -26,6 +26,12 @@ struct BoidConst {
   int reach_push;       // ceil(push_radius / h) particle cells
 };
 
+struct ObstacleConst {  // N4: Obstacle Grid, D:C-OBST
+  float origin[3], cell;
+  int dims[3];
+  float w_obs, heavy;
+};
+
 struct McConst {
   float origin[3], spacing;
   uint32_t G;
@@ -37,7 +43,7 @@ struct McConst {
 enum KernelId {
   K_HASH_COUNT = 0, K_SCAN_CELLS, K_SCATTER, K_REORDER,          // particle grid
   K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
-  K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
+  K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_BOID_OBSTACLES, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
   K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_MC_EDGE_SCAN, K_MC_VERTICES, K_MC_EMIT_INDICES, K_ZERO_U32,
   K_NUM_KERNELS
 };
@@ -106,6 +112,8 @@ void launch_force_integrate(const SphConst& c, const BoidConst* bc, const GridBu
 void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                       uint32_t nb, const float* rhoS, const float* rho_bS, float4* bpos, float4* bvel,
                       float4* dv_parts, cudaStream_t s, Prof* prof);
+void launch_boid_obstacles(const ObstacleConst& oc, const float4* normals, const BoidConst& bc, const float4* bpos,
+                           float4* bvel, uint32_t nb, cudaStream_t s, Prof* prof);
 // mc.cu
 void upload_mc_tables();
 void mc_table_host(int8_t* tri, uint8_t* ntri);

@@ -148,7 +148,7 @@ def sphere_obstacle(space_min, space_max, cell, centre, radius, w_obs=0.05, heav
     """Synthetic Obstacle Grid (stands in for the paper's obstacle meshes): a grid of `cell`
     over the Boid Space whose cells within half a cell diagonal of the sphere's surface carry the outward unit normal of
     the sphere at the cell centre, all others zero.  Returns (obstacle params dict, normals (cells, 4) float32).
-    Input construction only: the avoidance rule itself lives in oracle/ and csrc/."""
+    Input construction only: no part of the avoidance rule is evaluated here."""
     lo = np.asarray(space_min, np.float64)
     hi = np.asarray(space_max, np.float64)
     dims = np.maximum(1, np.ceil((hi - lo) / cell)).astype(np.int64)

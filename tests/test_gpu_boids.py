@@ -92,3 +92,39 @@ def test_two_frames_free_running():
             out = sim.boid_step(cfg["boid"], dbp, dbv)
         bad, worst = vec_err(out["bvel"][:, :3], bvel[:, :3], rel=2e-5, abs_=2e-6)
         assert bad == 0, (bad, worst)
+
+
+# ---- N4: obstacle avoidance (P:261, P:336 step 7; D:C-OBST) ----------------------------------------------------------
+@pytest.mark.parametrize("idx,scale", [(1, None), (3, 2)])
+def test_boid_step_with_obstacle_grid_matches_oracle(idx, scale):
+    import torch
+    from paper_2311_15088_b200 import binding as B
+    cfg = W.config(idx, scale=scale)
+    bp = cfg["boid"]
+    lo, hi = np.array(bp["space_min"]), np.array(bp["space_max"])
+    centre = cfg["bpos"][:, :3].mean(axis=0).astype(np.float64)  # an obstacle in the middle of the swarm
+    op, normals = W.sphere_obstacle(lo, hi, 0.6 * bp["visible_range"], centre, 0.8 * bp["visible_range"],
+                                    w_obs=0.07, heavy=2.5)
+    ref = R.step(cfg["sph"], cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"], bp)
+    refb = R.boid_step(cfg["sph"], bp, cfg["pos"], cfg["vel"], ref["density"], cfg["bpos"], cfg["bvel"])
+    want = R.boid_obstacles(op, normals, bp["protect_range"], bp["visible_range"], refb["bpos"], refb["bvel"])
+    assert (want != refb["bvel"]).any()  # the obstacle really acts on some boids
+    with Sim(cfg) as sim:
+        nrm = dev(normals)
+        B.boid_set_obstacles(sim.ctx, op, nrm)
+        pos, vel, bpos, bvel = dev(cfg["pos"]), dev(cfg["vel"]), dev(cfg["bpos"]), dev(cfg["bvel"])
+        sim.step(pos, vel, bpos, bvel, bp)
+        out = sim.boid_step(bp, bpos, bvel)
+        bad, worst = vec_err(out["bpos"][:, :3], refb["bpos"][:, :3])
+        assert bad == 0, ("bpos", bad, worst)
+        bad, worst = vec_err(out["bvel"][:, :3], want[:, :3])
+        assert bad == 0, ("bvel", bad, worst)
+        # untouched boids are bitwise the plain step's; cleared grid -> plain step again
+        same = (want == refb["bvel"]).all(axis=1)
+        B.boid_set_obstacles(sim.ctx, None, None)
+        pos, vel, bpos, bvel = dev(cfg["pos"]), dev(cfg["vel"]), dev(cfg["bpos"]), dev(cfg["bvel"])
+        sim.step(pos, vel, bpos, bvel, bp)
+        plain = sim.boid_step(bp, bpos, bvel)
+        assert np.array_equal(plain["bvel"][same], out["bvel"][same])
+        bad, worst = vec_err(plain["bvel"][:, :3], refb["bvel"][:, :3])
+        assert bad == 0
