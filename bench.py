@@ -275,6 +275,26 @@ def main():
     indexed = {"ms_per_pass": evi[0].elapsed_time(evi[1]) / 3, "vertices": n_iv, "triangles": n_tris,
                "what": "mc_extract_indexed: S14 + welded vertices, central-difference normals, index buffer"}
     del iverts, inorm, iidx
+    # N4 baseline (not part of `value`): neighbour counts through the sorted grid (grid build + count pass) against the
+    # paper's first, unsorted fixed-capacity hash grid, same positions, same counts
+    cnt_a = torch.zeros(n, dtype=torch.int32, device=fr.device)
+    cnt_b = torch.zeros(n, dtype=torch.int32, device=fr.device)
+    B.sph_neighbor_count(fr.ctx, fr.pos, cnt_a)
+    dropped = B.sph_hashgrid_neighbor_count(fr.ctx, fr.pos, 32, cnt_b)
+    evn = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    evn[0].record()
+    for _ in range(5):
+        B.sph_neighbor_count(fr.ctx, fr.pos, cnt_a)
+    evn[1].record()
+    for _ in range(5):
+        B.sph_hashgrid_neighbor_count(fr.ctx, fr.pos, 32, cnt_b, sync=False)
+    evn[2].record()
+    torch.cuda.synchronize()
+    nsearch = {"sorted_grid_us": 1e3 * evn[0].elapsed_time(evn[1]) / 5, "unsorted_hash_grid_us": 1e3 * evn[1].elapsed_time(evn[2]) / 5,
+               "max_per_cell": 32, "dropped": dropped, "counts_equal": bool((cnt_a == cnt_b).all().item()),
+               "what": "neighbour count of every particle: grid build + count pass (sph_neighbor_count) vs the paper's "
+                       "unsorted fixed-capacity hash grid (sph_hashgrid_neighbor_count)"}
+    del cnt_a, cnt_b
     # true neighbour pairs of that state (for the arithmetic roofline): one more SPH step with the count output
     ncount = torch.zeros(n, dtype=torch.int32, device=fr.device)
     B.sph_step(fr.ctx, fr.pos, fr.vel, fr.bpos, fr.bvel, cfg["boid"], ncount=ncount)
@@ -390,7 +410,7 @@ def main():
             "kernel_timing": {"how": "the same K frames run a second time with a CUDA event pair around every launch "
                                      "(on the launching stream); `value` comes from the first, un-instrumented run",
                               "ms_per_step_instrumented": 1e3 * t_profiled / K},
-            "indexed_mesh": indexed, "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "cpu_baseline": cpu,
+            "indexed_mesh": indexed, "neighbour_search_ab": nsearch, "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "cpu_baseline": cpu,
         }
         print(json.dumps(line))
     ranks.close()

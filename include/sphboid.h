@@ -120,6 +120,18 @@ typedef struct {
 } obstacle_params;
 int boid_set_obstacles(sph_ctx* ctx, const obstacle_params* op /* host */, const void* normals);
 
+/* S5-S6 without the density: the neighbour count of every particle (P:440-464 compute_neighbor_count; self counted,
+ * r^2 < h^2) through the sorted grid (builds it on pos first).  ncount = DEVICE u32[n], caller order. */
+int sph_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, void* stream, uint32_t* ncount);
+
+/* N4 baseline: the same counts through the paper's FIRST neighbour search (Listings 5-7):
+ * an unsorted hash_grid[cell * max_per_cell + slot] of particle ids filled with atomic slot counters, then the 27-cell
+ * walk reading positions through the ids.  Kept to measure the paper's claim that the sorted search is better
+ * (P:589).  A particle that finds its cell full is dropped (the paper leaves that case open); *dropped_host (host,
+ * optional; passing it synchronises) gets their number -- the counts equal sph_neighbor_count's iff it is 0. */
+int sph_hashgrid_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, uint32_t max_per_cell, void* stream,
+                                uint32_t* ncount, uint32_t* dropped_host);
+
 /* S8 has two kernels that compute the same forces: 0 (default) = the density pass stores each
  * particle's neighbour list (the paper's section 9 design) and the force pass reads it; 1 = the force pass
  * walks the 27 cells again.  Tests and A/B measurements force one. */

@@ -81,6 +81,8 @@ def lib():
         L.mc_voxel_sdf.argtypes = [_vp, _vp, _vp, _vp]
         L.mc_set_sdf_variant.argtypes = [_vp, C.c_int]
         L.boid_set_obstacles.argtypes = [_vp, _vp, _vp]
+        L.sph_neighbor_count.argtypes = [_vp, _vp, _u32, _vp, _vp]
+        L.sph_hashgrid_neighbor_count.argtypes = [_vp, _vp, _u32, _u32, _vp, _vp, _vp]
         L.sph_set_force_variant.argtypes = [_vp, C.c_int]
         L.mc_polygonise.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.mc_extract.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp]
@@ -102,7 +104,7 @@ def lib():
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "boid_set_obstacles", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
            "sph_profile_read", "sph_kernel_name"]
 
 
@@ -224,6 +226,20 @@ def boid_set_obstacles(ctx, op, normals):
         return _check(ctx, lib().boid_set_obstacles(ctx, None, None))
     o = _fill(ObstacleParams, op)
     return _check(ctx, lib().boid_set_obstacles(ctx, C.byref(o), _ptr(normals)))
+
+
+def sph_neighbor_count(ctx, pos, ncount, stream=None):
+    """Neighbour counts through the sorted grid (builds it on pos)."""
+    return _check(ctx, lib().sph_neighbor_count(ctx, _ptr(pos), pos.shape[0], _stream(stream), _ptr(ncount)))
+
+
+def sph_hashgrid_neighbor_count(ctx, pos, max_per_cell, ncount, stream=None, sync=True):
+    """N4 baseline: the same counts through the paper's unsorted fixed-capacity hash grid.  Returns the number of
+    particles dropped from full cells when sync."""
+    dropped = _u32(0)
+    _check(ctx, lib().sph_hashgrid_neighbor_count(ctx, _ptr(pos), pos.shape[0], int(max_per_cell), _stream(stream),
+                                                  _ptr(ncount), C.byref(dropped) if sync else None))
+    return int(dropped.value) if sync else None
 
 
 def sph_set_force_variant(ctx, variant):

@@ -43,6 +43,8 @@ struct sph_ctx {
   bool grid_fresh;       // pg holds a grid of (grid_pos, grid_n) and positions have not moved since
   bool step_state;       // pg/rhoS hold the step-start state of the last sph_step
   BoidConst bc;
+  uint32_t *hg_tracker, *hg_grid, *hg_dropped;  // N4 baseline: the paper's unsorted fixed-capacity hash grid (lazy)
+  uint32_t hg_cap;
   ObstacleConst oc;      // N4: Obstacle Grid set by boid_set_obstacles (normals stay caller-owned)
   const float4* obst_normals;
   bool boid_state;       // bg/rho_bS hold the boids given to the last sph_step
@@ -329,6 +331,7 @@ int sph_destroy(sph_ctx* ctx) {
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->ev_rho) cudaEventDestroy(ctx->ev_rho);
+  cudaFree(ctx->hg_tracker), cudaFree(ctx->hg_grid), cudaFree(ctx->hg_dropped);
   cudaFree(ctx->h_pos), cudaFree(ctx->h_vel), cudaFree(ctx->h_bpos), cudaFree(ctx->h_bvel), cudaFree(ctx->h_tris);
   delete ctx;
   return SPH_OK;
@@ -348,7 +351,7 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step", "k_boid_obstacles",
-    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32"};
+    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_hashgrid_fill", "k_hashgrid_count", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -532,6 +535,47 @@ int mc_set_sdf_variant(sph_ctx* ctx, int variant) {
   if (!ctx) return SPH_E_INVALID;
   if (variant < 0 || variant > 4) return fail(ctx, SPH_E_INVALID, "sdf variant must be 0..4");
   ctx->sdf_variant = variant;
+  return SPH_OK;
+}
+
+int sph_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, void* stream, uint32_t* ncount) {
+  if (!ctx) return SPH_E_INVALID;
+  if (n > ctx->p.max_particles) return fail(ctx, SPH_E_INVALID, "n exceeds max_particles");
+  if (n > 0 && (!pos || !aligned16(pos) || !ncount)) return fail(ctx, SPH_E_INVALID, "pos / ncount missing or misaligned");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  build_grid(ctx, pos, nullptr, n, s);
+  launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, nullptr, ncount, nullptr, s, &ctx->prof);
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+int sph_hashgrid_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, uint32_t max_per_cell, void* stream,
+                                uint32_t* ncount, uint32_t* dropped_host) {
+  if (!ctx) return SPH_E_INVALID;
+  if (n > ctx->p.max_particles) return fail(ctx, SPH_E_INVALID, "n exceeds max_particles");
+  if (max_per_cell == 0 || (uint64_t)max_per_cell * ctx->sc.grid.C > (1ull << 31))
+    return fail(ctx, SPH_E_INVALID, "max_per_cell out of range");
+  if (n > 0 && (!pos || !aligned16(pos) || !ncount)) return fail(ctx, SPH_E_INVALID, "pos / ncount missing or misaligned");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  if (!ctx->hg_tracker) {
+    CK(cudaMalloc(&ctx->hg_tracker, (size_t)ctx->sc.grid.C * 4));
+    CK(cudaMalloc(&ctx->hg_dropped, 4));
+  }
+  if (max_per_cell > ctx->hg_cap) {
+    cudaFree(ctx->hg_grid);
+    ctx->hg_grid = nullptr;
+    CK(cudaMalloc(&ctx->hg_grid, (size_t)ctx->sc.grid.C * max_per_cell * 4));
+    ctx->hg_cap = max_per_cell;
+  }
+  launch_hashgrid_count(ctx->sc.grid, ctx->sc.h2, (const float4*)pos, n, max_per_cell, ctx->hg_tracker, ctx->hg_grid,
+                        ctx->hg_dropped, ncount, s, &ctx->prof);
+  CK(cudaGetLastError());
+  if (dropped_host) {
+    CK(cudaMemcpyAsync(dropped_host, ctx->hg_dropped, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+  }
   return SPH_OK;
 }
 

@@ -168,6 +168,53 @@ __global__ void __launch_bounds__(kThreads) k_reorder(const uint32_t* __restrict
   if (vel) velS[dst] = __ldg(vel + id);
 }
 
+// ---- N4: the paper's FIRST neighbour search, kept as a measured baseline (K7) -------------
+// compute_hash_grid (Listing 5): hash_grid[cell * max_per_cell + slot] = particle id, slot = the cell's running count
+// (hash_grid_tracker).  Particles that find their cell full are dropped and counted (the paper leaves that case open).
+__global__ void __launch_bounds__(kThreads) k_hashgrid_fill(GridDesc g, const float4* __restrict__ pos, uint32_t n,
+                                                            uint32_t cap, uint32_t* __restrict__ tracker,
+                                                            uint32_t* __restrict__ hash_grid,
+                                                            uint32_t* __restrict__ dropped) {
+  const uint32_t i = blockIdx.x * kThreads + threadIdx.x;
+  if (i >= n) return;
+  const float4 p = __ldg(pos + i);
+  const uint32_t k = cell_hash(g, cell_coord(p.x, g.lo[0], g.cell, g.dim[0]), cell_coord(p.y, g.lo[1], g.cell, g.dim[1]),
+                               cell_coord(p.z, g.lo[2], g.cell, g.dim[2]));
+  const uint32_t slot = atomicAdd(tracker + k, 1u);
+  if (slot < cap)
+    hash_grid[(size_t)k * cap + slot] = i;
+  else
+    atomicAdd(dropped, 1u);
+}
+
+// compute_neighbor_list (Listings 6-7) reduced to its count: the 27 cells around the particle's own (cells outside the
+// grid skipped, D:A-BOUND), every stored id a potential neighbour read through the index, r^2 < h^2.
+__global__ void __launch_bounds__(kThreads) k_hashgrid_count(GridDesc g, float h2, const float4* __restrict__ pos,
+                                                             uint32_t n, uint32_t cap,
+                                                             const uint32_t* __restrict__ tracker,
+                                                             const uint32_t* __restrict__ hash_grid,
+                                                             uint32_t* __restrict__ ncount) {
+  const uint32_t i = blockIdx.x * kThreads + threadIdx.x;
+  if (i >= n) return;
+  const float4 pi = __ldg(pos + i);
+  const int cx = cell_coord(pi.x, g.lo[0], g.cell, g.dim[0]);
+  const int cy = cell_coord(pi.y, g.lo[1], g.cell, g.dim[1]);
+  const int cz = cell_coord(pi.z, g.lo[2], g.cell, g.dim[2]);
+  uint32_t cnt = 0;
+  for (int z = max(cz - 1, 0); z <= min(cz + 1, g.dim[2] - 1); ++z)
+    for (int y = max(cy - 1, 0); y <= min(cy + 1, g.dim[1] - 1); ++y)
+      for (int x = max(cx - 1, 0); x <= min(cx + 1, g.dim[0] - 1); ++x) {
+        const uint32_t k = cell_hash(g, x, y, z);
+        const uint32_t m = min(__ldg(tracker + k), cap);
+        const uint32_t* ids = hash_grid + (size_t)k * cap;
+        for (uint32_t j = 0; j < m; ++j) {
+          const float4 pj = __ldg(pos + __ldg(ids + j));
+          cnt += dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z) < h2 ? 1u : 0u;
+        }
+      }
+  ncount[i] = cnt;
+}
+
 }  // namespace
 
 uint32_t grid_scan_tiles(uint32_t C) { return (C + 1 + kScanTile - 1) / kScanTile; }
@@ -199,6 +246,20 @@ void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const f
   }
   b.aabb_now = b.aabb + 6 * b.slot;
   b.slot ^= 1;
+}
+
+void launch_hashgrid_count(const GridDesc& g, float h2, const float4* pos, uint32_t n, uint32_t cap, uint32_t* tracker,
+                           uint32_t* hash_grid, uint32_t* dropped, uint32_t* ncount, cudaStream_t s, Prof* prof) {
+  cudaMemsetAsync(tracker, 0, (size_t)g.C * 4, s);
+  cudaMemsetAsync(dropped, 0, 4, s);
+  if (n == 0) return;
+  const uint32_t blocks = (n + kThreads - 1) / kThreads;
+  prof->begin(K_HASHGRID_FILL, s);
+  k_hashgrid_fill<<<blocks, kThreads, 0, s>>>(g, pos, n, cap, tracker, hash_grid, dropped);
+  prof->end(s);
+  prof->begin(K_HASHGRID_COUNT, s);
+  k_hashgrid_count<<<blocks, kThreads, 0, s>>>(g, h2, pos, n, cap, tracker, hash_grid, ncount);
+  prof->end(s);
 }
 
 }  // namespace sphb

@@ -6,7 +6,7 @@ import torch
 from oracle import refbind as R
 from paper_2311_15088_b200 import binding as B
 from paper_2311_15088_b200 import workloads as W
-from tests.gpuutil import Sim, dev
+from tests.gpuutil import Sim, dev, host_u32
 
 pytestmark = pytest.mark.gpu
 
@@ -63,3 +63,25 @@ def test_grid_rebuild_is_repeatable():
         for _ in range(5):
             again = sim.build_grid(pos)
             assert all(np.array_equal(a, b) for a, b in zip(first, again))
+
+
+# ---- neighbour counts: sorted grid vs the paper's unsorted fixed-capacity hash grid (N4 baseline) ----------
+@pytest.mark.parametrize("idx,scale", [(1, None), (2, None), (4, 4), (5, 4)])
+def test_neighbor_counts_sorted_and_hashgrid_match_oracle(idx, scale):
+    import torch
+    from oracle import refbind as R
+    from paper_2311_15088_b200 import binding as B
+    cfg = W.config(idx, scale=scale)
+    _, ref_cnt = R.density(cfg["sph"], cfg["pos"])
+    with Sim(cfg) as sim:
+        pos = dev(cfg["pos"])
+        cnt = torch.zeros(cfg["n"], dtype=torch.int32, device="cuda")
+        B.sph_neighbor_count(sim.ctx, pos, cnt)
+        assert np.array_equal(host_u32(cnt), ref_cnt)
+        cnt.zero_()
+        dropped = B.sph_hashgrid_neighbor_count(sim.ctx, pos, 64, cnt)
+        assert dropped == 0 and np.array_equal(host_u32(cnt), ref_cnt)
+        # a capacity below the fullest cell: particles are dropped, reported, and the counts can only shrink
+        cnt2 = torch.zeros_like(cnt)
+        dropped = B.sph_hashgrid_neighbor_count(sim.ctx, pos, 4, cnt2)
+        assert dropped > 0 and bool((cnt2 <= cnt).all()) and bool((cnt2 < cnt).any())
