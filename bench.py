@@ -170,6 +170,62 @@ def run_reference(args, cfg_idx):
     print(json.dumps(line))
 
 
+def run_slab(args):
+    """--decomposition slab (N2): the fluid of the workload cut into slabs over the ranks, strong scaling; SPH step only
+    (boids and the surface pass are not decomposed).  Exchange: neighbour send / receive over NCCL."""
+    import torch
+    from paper_2311_15088_b200 import binding as B
+    from paper_2311_15088_b200 import dist as D
+    from paper_2311_15088_b200 import slab as S
+    from paper_2311_15088_b200 import workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    B.lib()
+    ranks = D.Ranks()
+    dev = ranks.local_rank
+    torch.cuda.set_device(dev)
+    cfg = W.config(args.config)
+    n, K = cfg["n"], args.steps
+    lay = S.SlabLayout(cfg["sph"], ranks.world)
+    p, v = S.split_initial(lay, cfg["pos"], cfg["vel"])[ranks.rank]
+    be = S.GpuBackend(cfg["sph"], min(n, 2 * (n // ranks.world) + (1 << 16)), device=dev)
+    ex = (S.DistExchange(ranks.dist, ranks.rank, ranks.world, torch.device("cuda", dev)) if ranks.world > 1
+          else S.LoopbackExchange(1))
+    sim = S.SlabSim(lay, ranks.rank, be, ex, be.to_device(p), be.to_device(v))
+    for _ in range(max(args.warmup, 3)):
+        sim.step()
+    sampler = ClockSampler(dev)
+    sampler.start()
+    time.sleep(0.15)
+    ranks.barrier()
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    launches0 = B.sph_launch_count(be.ctx)
+    ev[0].record()
+    for _ in range(K):
+        sim.step()
+    ev[1].record()
+    torch.cuda.synchronize()
+    ranks.barrier()
+    t = ev[0].elapsed_time(ev[1]) * 1e-3
+    launches = B.sph_launch_count(be.ctx) - launches0
+    clocks = sampler.stop()
+    t_max, _ = ranks.combine(t, 0.0)
+    owned = ranks.reduce_max([float(sim.n_owned), float(sim.stats["ghosts"])])
+    if ranks.rank == 0:
+        print(json.dumps({
+            "metric": "particle-updates/s (SPH step of the fluid, slab-decomposed over the ranks; no boids, no surface pass)",
+            "value": n * K / t_max, "unit": "particle-updates/s", "n_gpus": ranks.world, "steps": K,
+            "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_max / K, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg["name"], "particles": n, "parallelism": "slab x%d along axis %d" % (ranks.world, lay.axis),
+                       "max_owned_per_rank": int(owned[0]), "max_ghosts_per_rank": int(owned[1]),
+                       "exchange": "2 neighbour send/recv pairs per step (halo of 2 h, migration), NCCL"},
+            "gpu_launches": launches, "clocks": clocks, "e2e": None, "roofline": None, "cpu_baseline": None}))
+    be.close()
+    ranks.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -181,9 +237,13 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--force-variant", type=int, default=0, help="A/B: 0 = stored neighbour masks (default), 1 = grid walk")
     ap.add_argument("--sdf-variant", type=int, default=0, help="A/B: 0 = cost model (default), 1-4 force one S14 kernel")
+    ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default) or the fluid cut into slabs with halo exchange (N2, SPH step only)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args, args.config)
+    if args.decomposition == "slab":
+        return run_slab(args)
     if args.warmup < 3:
         args.warmup = 3
 

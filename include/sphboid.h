@@ -120,6 +120,14 @@ typedef struct {
 } obstacle_params;
 int boid_set_obstacles(sph_ctx* ctx, const obstacle_params* op /* host */, const void* normals);
 
+/* N2 (the paper only names a multi-node decomposition as future work): support for
+ * a slab decomposition.  Copies, in ascending index order, the particles with lo <= pos[axis] < hi (use -INFINITY /
+ * INFINITY for an open side) to out_pos / out_vel (DEVICE float4[capacity]; vel / out_vel may both be NULL).
+ * *count_host (host, optional; passing it synchronises) gets the number selected; SPH_E_CAPACITY if it exceeds capacity
+ * (nothing past capacity is written). */
+int sph_pack_range(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, int axis, float lo, float hi, void* stream,
+                   void* out_pos, void* out_vel, uint32_t capacity, uint32_t* count_host);
+
 /* S5-S6 without the density: the neighbour count of every particle (P:440-464 compute_neighbor_count; self counted,
  * r^2 < h^2) through the sorted grid (builds it on pos first).  ncount = DEVICE u32[n], caller order. */
 int sph_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, void* stream, uint32_t* ncount);

@@ -82,6 +82,7 @@ def lib():
         L.mc_set_sdf_variant.argtypes = [_vp, C.c_int]
         L.boid_set_obstacles.argtypes = [_vp, _vp, _vp]
         L.sph_neighbor_count.argtypes = [_vp, _vp, _u32, _vp, _vp]
+        L.sph_pack_range.argtypes = [_vp, _vp, _vp, _u32, C.c_int, _f, _f, _vp, _vp, _vp, _u32, _vp]
         L.sph_hashgrid_neighbor_count.argtypes = [_vp, _vp, _u32, _u32, _vp, _vp, _vp]
         L.sph_set_force_variant.argtypes = [_vp, C.c_int]
         L.mc_polygonise.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp, _vp]
@@ -104,7 +105,7 @@ def lib():
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_pack_range", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
            "sph_profile_read", "sph_kernel_name"]
 
 
@@ -226,6 +227,15 @@ def boid_set_obstacles(ctx, op, normals):
         return _check(ctx, lib().boid_set_obstacles(ctx, None, None))
     o = _fill(ObstacleParams, op)
     return _check(ctx, lib().boid_set_obstacles(ctx, C.byref(o), _ptr(normals)))
+
+
+def sph_pack_range(ctx, pos, vel, n, axis, lo, hi, out_pos, out_vel, stream=None):
+    """N2: ordered copy of the particles with lo <= pos[axis] < hi among the first n; returns their number."""
+    cnt = _u32(0)
+    rc = lib().sph_pack_range(ctx, _ptr(pos), _ptr(vel), int(n), int(axis), float(lo), float(hi), _stream(stream),
+                              _ptr(out_pos), _ptr(out_vel), 0 if out_pos is None else out_pos.shape[0], C.byref(cnt))
+    _check(ctx, rc)
+    return int(cnt.value)
 
 
 def sph_neighbor_count(ctx, pos, ncount, stream=None):

@@ -43,6 +43,7 @@ struct sph_ctx {
   bool grid_fresh;       // pg holds a grid of (grid_pos, grid_n) and positions have not moved since
   bool step_state;       // pg/rhoS hold the step-start state of the last sph_step
   BoidConst bc;
+  uint32_t *pack_blocks, *pack_total;  // N2: scratch of sph_pack_range (lazy)
   uint32_t *hg_tracker, *hg_grid, *hg_dropped;  // N4 baseline: the paper's unsorted fixed-capacity hash grid (lazy)
   uint32_t hg_cap;
   ObstacleConst oc;      // N4: Obstacle Grid set by boid_set_obstacles (normals stay caller-owned)
@@ -332,6 +333,7 @@ int sph_destroy(sph_ctx* ctx) {
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->ev_rho) cudaEventDestroy(ctx->ev_rho);
   cudaFree(ctx->hg_tracker), cudaFree(ctx->hg_grid), cudaFree(ctx->hg_dropped);
+  cudaFree(ctx->pack_blocks), cudaFree(ctx->pack_total);
   cudaFree(ctx->h_pos), cudaFree(ctx->h_vel), cudaFree(ctx->h_bpos), cudaFree(ctx->h_bvel), cudaFree(ctx->h_tris);
   delete ctx;
   return SPH_OK;
@@ -351,7 +353,7 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step", "k_boid_obstacles",
-    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_hashgrid_fill", "k_hashgrid_count", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32"};
+    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_hashgrid_fill", "k_hashgrid_count", "k_range_count", "k_range_scan", "k_range_scatter", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -535,6 +537,31 @@ int mc_set_sdf_variant(sph_ctx* ctx, int variant) {
   if (!ctx) return SPH_E_INVALID;
   if (variant < 0 || variant > 4) return fail(ctx, SPH_E_INVALID, "sdf variant must be 0..4");
   ctx->sdf_variant = variant;
+  return SPH_OK;
+}
+
+int sph_pack_range(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, int axis, float lo, float hi, void* stream,
+                   void* out_pos, void* out_vel, uint32_t capacity, uint32_t* count_host) {
+  if (!ctx) return SPH_E_INVALID;
+  if (axis < 0 || axis > 2) return fail(ctx, SPH_E_INVALID, "axis must be 0, 1 or 2");
+  if (n > ctx->p.max_particles) return fail(ctx, SPH_E_INVALID, "n exceeds max_particles");
+  if (n > 0 && (!pos || !aligned16(pos) || !aligned16(vel) || !aligned16(out_pos) || !aligned16(out_vel) ||
+                (capacity > 0 && !out_pos) || (vel && capacity > 0 && !out_vel)))
+    return fail(ctx, SPH_E_INVALID, "pos / out arrays missing or misaligned");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  if (!ctx->pack_blocks) {
+    CK(cudaMalloc(&ctx->pack_blocks, ((size_t)ctx->p.max_particles / 256 + 2) * 4));
+    CK(cudaMalloc(&ctx->pack_total, 4));
+  }
+  launch_pack_range((const float4*)pos, (const float4*)vel, n, axis, lo, hi, ctx->pack_blocks, ctx->pack_total,
+                    (float4*)out_pos, (float4*)out_vel, capacity, s, &ctx->prof);
+  CK(cudaGetLastError());
+  if (count_host) {
+    CK(cudaMemcpyAsync(count_host, ctx->pack_total, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    if (*count_host > capacity) return fail(ctx, SPH_E_CAPACITY, "pack buffer too small");
+  }
   return SPH_OK;
 }
 

@@ -215,6 +215,59 @@ __global__ void __launch_bounds__(kThreads) k_hashgrid_count(GridDesc g, float h
   ncount[i] = cnt;
 }
 
+// ---- N2: slab decomposition support -- ordered selection of the particles of a coordinate range --
+// select_i = lo <= pos_i[axis] < hi.  Three small kernels: per-block counts, one-block exclusive scan of the counts,
+// per-block ordered scatter; the output keeps ascending particle index, so a decomposed run is reproducible.
+__device__ __forceinline__ bool in_range(const float4& p, int axis, float lo, float hi) {
+  const float x = axis == 0 ? p.x : (axis == 1 ? p.y : p.z);
+  return x >= lo && x < hi;
+}
+
+__global__ void __launch_bounds__(kThreads) k_range_count(const float4* __restrict__ pos, uint32_t n, int axis, float lo,
+                                                          float hi, uint32_t* __restrict__ block_count) {
+  const uint32_t i = blockIdx.x * kThreads + threadIdx.x;
+  const bool sel = i < n && in_range(__ldg(pos + i), axis, lo, hi);
+  const uint32_t c = __syncthreads_count(sel);
+  if (threadIdx.x == 0) block_count[blockIdx.x] = c;
+}
+
+__global__ void __launch_bounds__(1024) k_range_scan(uint32_t* __restrict__ block_count, uint32_t nb,
+                                                     uint32_t* __restrict__ total) {
+  __shared__ uint32_t s_scan[33];
+  uint32_t carry = 0;
+  for (uint32_t base = 0; base < nb; base += 1024) {
+    const uint32_t j = base + threadIdx.x;
+    const uint32_t v = j < nb ? block_count[j] : 0u;
+    uint32_t sum;
+    const uint32_t ex = block_exclusive_scan(v, s_scan, &sum);
+    if (j < nb) block_count[j] = carry + ex;
+    carry += sum;
+  }
+  if (threadIdx.x == 0) *total = carry;
+}
+
+__global__ void __launch_bounds__(kThreads) k_range_scatter(const float4* __restrict__ pos, const float4* __restrict__ vel,
+                                                            uint32_t n, int axis, float lo, float hi,
+                                                            const uint32_t* __restrict__ block_offset,
+                                                            float4* __restrict__ out_pos, float4* __restrict__ out_vel,
+                                                            uint32_t capacity) {
+  __shared__ uint32_t s_scan[33];
+  const uint32_t i = blockIdx.x * kThreads + threadIdx.x;
+  float4 p = make_float4(0.f, 0.f, 0.f, 0.f);
+  bool sel = false;
+  if (i < n) {
+    p = __ldg(pos + i);
+    sel = in_range(p, axis, lo, hi);
+  }
+  uint32_t total;
+  const uint32_t ex = block_exclusive_scan(sel ? 1u : 0u, s_scan, &total);
+  const uint32_t dst = block_offset[blockIdx.x] + ex;
+  if (sel && dst < capacity) {
+    out_pos[dst] = p;
+    if (vel) out_vel[dst] = __ldg(vel + i);
+  }
+}
+
 }  // namespace
 
 uint32_t grid_scan_tiles(uint32_t C) { return (C + 1 + kScanTile - 1) / kScanTile; }
@@ -259,6 +312,25 @@ void launch_hashgrid_count(const GridDesc& g, float h2, const float4* pos, uint3
   prof->end(s);
   prof->begin(K_HASHGRID_COUNT, s);
   k_hashgrid_count<<<blocks, kThreads, 0, s>>>(g, h2, pos, n, cap, tracker, hash_grid, ncount);
+  prof->end(s);
+}
+
+void launch_pack_range(const float4* pos, const float4* vel, uint32_t n, int axis, float lo, float hi,
+                       uint32_t* block_count, uint32_t* total_dev, float4* out_pos, float4* out_vel, uint32_t capacity,
+                       cudaStream_t s, Prof* prof) {
+  const uint32_t blocks = (n + kThreads - 1) / kThreads;
+  if (blocks == 0) {
+    cudaMemsetAsync(total_dev, 0, 4, s);
+    return;
+  }
+  prof->begin(K_RANGE_COUNT, s);
+  k_range_count<<<blocks, kThreads, 0, s>>>(pos, n, axis, lo, hi, block_count);
+  prof->end(s);
+  prof->begin(K_RANGE_SCAN, s);
+  k_range_scan<<<1, 1024, 0, s>>>(block_count, blocks, total_dev);
+  prof->end(s);
+  prof->begin(K_RANGE_SCATTER, s);
+  k_range_scatter<<<blocks, kThreads, 0, s>>>(pos, vel, n, axis, lo, hi, block_count, out_pos, out_vel, capacity);
   prof->end(s);
 }
 

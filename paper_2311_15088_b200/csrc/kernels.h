@@ -44,7 +44,7 @@ enum KernelId {
   K_HASH_COUNT = 0, K_SCAN_CELLS, K_SCATTER, K_REORDER,          // particle grid
   K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
   K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_BOID_OBSTACLES, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
-  K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_HASHGRID_FILL, K_HASHGRID_COUNT, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_MC_EDGE_SCAN, K_MC_VERTICES, K_MC_EMIT_INDICES, K_ZERO_U32,
+  K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_HASHGRID_FILL, K_HASHGRID_COUNT, K_RANGE_COUNT, K_RANGE_SCAN, K_RANGE_SCATTER, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_MC_EDGE_SCAN, K_MC_VERTICES, K_MC_EMIT_INDICES, K_ZERO_U32,
   K_NUM_KERNELS
 };
 
@@ -98,6 +98,9 @@ struct SdfPlan {
 void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
                        ScanState& scan, cudaStream_t s, Prof* prof, bool boid_grid);
 uint32_t grid_scan_tiles(uint32_t C);
+void launch_pack_range(const float4* pos, const float4* vel, uint32_t n, int axis, float lo, float hi,
+                       uint32_t* block_count, uint32_t* total_dev, float4* out_pos, float4* out_vel, uint32_t capacity,
+                       cudaStream_t s, Prof* prof);
 void launch_hashgrid_count(const GridDesc& g, float h2, const float4* pos, uint32_t n, uint32_t cap, uint32_t* tracker,
                            uint32_t* hash_grid, uint32_t* dropped, uint32_t* ncount, cudaStream_t s, Prof* prof);
 // sph.cu

@@ -1,8 +1,7 @@
-"""Multi-GPU plumbing: one process per GPU, "replicas only".
+"""Multi-GPU plumbing: one process per GPU.
 
-The single-GPU pipeline does not shard without a halo exchange (not built),
-so `bench.py --gpus N` runs N independent replicas of the workload, one per rank, with no data-path
-collective.  torch.distributed is used only for the barrier around the timed region and for combining the
+By default `bench.py --gpus N` runs N independent replicas of the workload, one per rank, with no data-path
+collective (the slab decomposition of the SPH step, with its neighbour halo exchange, lives in slab.py).  torch.distributed is used only for the barrier around the timed region and for combining the
 per-rank results: time = max over ranks, units = sum over ranks.
 """
 import os

@@ -1,0 +1,236 @@
+"""N2 (SURVEY.md sections 8(e), 8(f)): slab decomposition of the SPH step over ranks, one process per GPU.
+
+The paper runs on one GPU and only names a multi-node decomposition as future work; the
+scheme here is the standard one for a short-range particle method:
+
+* the box is cut into slabs along its longest axis, at cell boundaries (multiples of h from box_min); rank r owns the
+  particles with lo_r <= x < hi_r, the outermost slabs being open towards -inf / +inf (particles clamped onto a wall
+  or started outside the box still have an owner);
+* every step each rank receives, from its two neighbours, copies of their particles within 2 h of the shared face
+  ("ghosts": the force on an owned particle needs rho of its neighbours within h, and the rho of those needs THEIR
+  neighbours within another h), runs the unmodified single-GPU step (sph_step through the C ABI) on
+  [owned | ghosts], and keeps the first n_owned results -- an owned particle sees exactly the neighbour set of the
+  undecomposed run, so its new state is that run's up to the order of the binary64 sums;
+* owned particles that crossed a face migrate to the neighbour.
+
+Exchange steps: two neighbour send / receive pairs per step (halo, migration), variable-size; no global collective.
+This module is orchestration only: selection and packing run in libsphboid (sph_pack_range), the step is sph_step,
+torch.distributed (NCCL on GPUs, gloo in the CPU tests) moves the packed buffers.  Boids and the surface pass are not
+decomposed here (boids would be replicated with an all-reduce of the fluid->boid force; the voxel grid would be cut
+along the same axis): the decomposed run is fluid only.
+
+The exchange is pluggable (`Exchange`): `DistExchange` uses torch.distributed; `LoopbackExchange` connects several
+domains inside ONE process (the single-GPU emulation the GPU test uses: ranks run one after the other, never
+concurrently waiting on each other).
+"""
+import math
+
+import numpy as np
+
+
+class SlabLayout:
+    """Which rank owns which x-range (pure host logic, no device)."""
+
+    def __init__(self, sph, world, axis=None):
+        lo, hi = np.asarray(sph["box_min"], np.float64), np.asarray(sph["box_max"], np.float64)
+        self.h = float(sph["h"])
+        self.axis = int(np.argmax(hi - lo)) if axis is None else int(axis)
+        self.world = int(world)
+        self.dim = max(1, int(math.ceil((hi[self.axis] - lo[self.axis]) / self.h)))
+        self.cells_per_rank = int(math.ceil(self.dim / self.world))
+        if self.world > 1 and self.cells_per_rank < 2:
+            raise ValueError("slabs must be at least 2 h wide (ghost layers of neighbours must not overlap)")
+        self.origin = float(np.float32(lo[self.axis]))
+        # faces in binary32, the precision positions are compared in
+        self.faces = [float(np.float32(self.origin + np.float32(self.cells_per_rank * r) * np.float32(self.h)))
+                      for r in range(1, self.world)]
+
+    def bounds(self, rank):
+        """[lo, hi) of rank's slab; the outermost slabs are open."""
+        lo = -math.inf if rank == 0 else self.faces[rank - 1]
+        hi = math.inf if rank == self.world - 1 else self.faces[rank]
+        return lo, hi
+
+    def owner(self, x):
+        """Rank that owns coordinate(s) x (numpy, binary32 comparison)."""
+        x = np.asarray(x, np.float32)
+        return np.searchsorted(np.asarray(self.faces, np.float32), x, side="right").astype(np.int64)
+
+    def halo_width(self):
+        return float(np.float32(2.0) * np.float32(self.h))
+
+
+class LoopbackExchange:
+    """Connects the domains of ONE process: a two-phase exchange (everybody posts, then everybody collects), so the
+    emulated ranks run one after the other and never wait on each other."""
+
+    def __init__(self, world):
+        self.world = world
+        self.box = {}
+
+    def post(self, rank, tag, to_left, to_right):
+        """to_left / to_right: (pos, vel) tensors or None."""
+        if rank > 0 and to_left is not None:
+            self.box[(rank - 1, tag, "from_right")] = to_left
+        if rank < self.world - 1 and to_right is not None:
+            self.box[(rank + 1, tag, "from_left")] = to_right
+
+    def collect(self, rank, tag):
+        return self.box.pop((rank, tag, "from_left"), None), self.box.pop((rank, tag, "from_right"), None)
+
+
+class DistExchange:
+    """torch.distributed neighbour exchange (NCCL on GPUs, gloo on CPU tensors): counts first, then the payloads."""
+
+    def __init__(self, dist, rank, world, device):
+        self.dist, self.rank, self.world, self.device = dist, rank, world, device
+        self.pending = {}
+
+    def post(self, rank, tag, to_left, to_right):
+        self.pending[tag] = (to_left, to_right)
+
+    def collect(self, rank, tag):
+        import torch
+        to_left, to_right = self.pending.pop(tag)
+        dist = self.dist
+        left, right = rank - 1, rank + 1
+        has_l, has_r = rank > 0, rank < self.world - 1
+
+        def count(t):
+            return torch.tensor([0 if t is None else t[0].shape[0]], dtype=torch.int64, device=self.device)
+
+        n_from = {"l": torch.zeros(1, dtype=torch.int64, device=self.device),
+                  "r": torch.zeros(1, dtype=torch.int64, device=self.device)}
+        ops = []
+        if has_l:
+            ops += [dist.P2POp(dist.isend, count(to_left), left), dist.P2POp(dist.irecv, n_from["l"], left)]
+        if has_r:
+            ops += [dist.P2POp(dist.isend, count(to_right), right), dist.P2POp(dist.irecv, n_from["r"], right)]
+        for w in (dist.batch_isend_irecv(ops) if ops else []):
+            w.wait()
+        nl, nr = int(n_from["l"].item()), int(n_from["r"].item())
+        like = to_left if to_left is not None else to_right
+        dtype = like[0].dtype if like is not None else torch.float32
+        recv_l = (torch.empty(nl, 4, dtype=dtype, device=self.device), torch.empty(nl, 4, dtype=dtype, device=self.device))
+        recv_r = (torch.empty(nr, 4, dtype=dtype, device=self.device), torch.empty(nr, 4, dtype=dtype, device=self.device))
+        ops = []
+        if has_l:
+            if to_left is not None and to_left[0].shape[0]:
+                ops += [dist.P2POp(dist.isend, to_left[0].contiguous(), left), dist.P2POp(dist.isend, to_left[1].contiguous(), left)]
+            if nl:
+                ops += [dist.P2POp(dist.irecv, recv_l[0], left), dist.P2POp(dist.irecv, recv_l[1], left)]
+        if has_r:
+            if to_right is not None and to_right[0].shape[0]:
+                ops += [dist.P2POp(dist.isend, to_right[0].contiguous(), right), dist.P2POp(dist.isend, to_right[1].contiguous(), right)]
+            if nr:
+                ops += [dist.P2POp(dist.irecv, recv_r[0], right), dist.P2POp(dist.irecv, recv_r[1], right)]
+        for w in (dist.batch_isend_irecv(ops) if ops else []):
+            w.wait()
+        return (recv_l if nl else None), (recv_r if nr else None)
+
+
+class GpuBackend:
+    """Selection and stepping through libsphboid on one GPU (device memory from torch)."""
+
+    def __init__(self, sph, capacity, device=0):
+        import torch
+        from . import binding as B
+        self.B, self.torch = B, torch
+        self.device = torch.device("cuda", device)
+        torch.cuda.set_device(self.device)
+        self.capacity = int(capacity)
+        self.ctx = B.sph_create(sph, self.capacity, 1, 0, device=device)
+        self.scratch = [torch.empty(self.capacity, 4, device=self.device) for _ in range(2)]
+
+    def to_device(self, a):
+        return self.torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(self.device)
+
+    def pack(self, pos, vel, n, axis, lo, hi):
+        """Ordered copy of the particles of the first n with lo <= x < hi -> (pos, vel) tensors (fresh storage)."""
+        k = self.B.sph_pack_range(self.ctx, pos, vel, n, axis, lo, hi, self.scratch[0], self.scratch[1])
+        return self.scratch[0][:k].clone(), self.scratch[1][:k].clone()
+
+    def step(self, pos, vel):
+        self.B.sph_step(self.ctx, pos, vel)
+
+    def cat(self, parts):
+        return self.torch.cat(parts, 0) if len(parts) > 1 else parts[0]
+
+    def close(self):
+        if self.ctx is not None:
+            self.B.sph_destroy(self.ctx)
+            self.ctx = None
+
+
+class SlabSim:
+    """One rank of the decomposed fluid.  pos / vel: this rank's OWNED particles ((n, 4) tensors of the backend)."""
+
+    def __init__(self, layout, rank, backend, exchange, pos, vel):
+        self.layout, self.rank, self.backend, self.exchange = layout, rank, backend, exchange
+        self.lo, self.hi = layout.bounds(rank)
+        self.pos, self.vel = pos, vel
+        self.n_owned = pos.shape[0]
+        self.halo = layout.halo_width() * 1.001  # a little over 2 h: the pair predicate is evaluated in binary32
+        self.step_no = 0
+        self.stats = dict(ghosts=0, migrated_out=0)
+
+    # -- phase 1: halo ---------------------------------------------------------------------------------------------
+    def post_halo(self):
+        ax, be = self.layout.axis, self.backend
+        to_left = be.pack(self.pos, self.vel, self.n_owned, ax, self.lo, self.lo + self.halo) if self.rank > 0 else None
+        to_right = (be.pack(self.pos, self.vel, self.n_owned, ax, self.hi - self.halo, self.hi)
+                    if self.rank < self.layout.world - 1 else None)
+        self.exchange.post(self.rank, ("halo", self.step_no), to_left, to_right)
+
+    def step_with_halo(self):
+        from_left, from_right = self.exchange.collect(self.rank, ("halo", self.step_no))
+        ghosts = [g for g in (from_left, from_right) if g is not None and g[0].shape[0] > 0]
+        pos_all = self.backend.cat([self.pos] + [g[0] for g in ghosts])
+        vel_all = self.backend.cat([self.vel] + [g[1] for g in ghosts])
+        self.stats["ghosts"] = pos_all.shape[0] - self.n_owned
+        self.backend.step(pos_all, vel_all)  # in place; the ghosts' results are not used
+        self.pos, self.vel = pos_all[:self.n_owned], vel_all[:self.n_owned]
+
+    # -- phase 2: migration ----------------------------------------------------------------------------------------
+    def post_migration(self):
+        ax, be = self.layout.axis, self.backend
+        inf = math.inf
+        go_left = be.pack(self.pos, self.vel, self.n_owned, ax, -inf, self.lo) if self.rank > 0 else None
+        go_right = be.pack(self.pos, self.vel, self.n_owned, ax, self.hi, inf) if self.rank < self.layout.world - 1 else None
+        self._stay = be.pack(self.pos, self.vel, self.n_owned, ax, self.lo, self.hi)
+        self.stats["migrated_out"] = self.n_owned - self._stay[0].shape[0]
+        self.exchange.post(self.rank, ("move", self.step_no), go_left, go_right)
+
+    def finish_migration(self):
+        from_left, from_right = self.exchange.collect(self.rank, ("move", self.step_no))
+        parts = [self._stay] + [g for g in (from_left, from_right) if g is not None and g[0].shape[0] > 0]
+        self.pos = self.backend.cat([p[0] for p in parts])
+        self.vel = self.backend.cat([p[1] for p in parts])
+        self.n_owned = self.pos.shape[0]
+        self.step_no += 1
+
+    def step(self):
+        """One decomposed step (with DistExchange every rank calls this; with LoopbackExchange drive the phases)."""
+        self.post_halo()
+        self.step_with_halo()
+        self.post_migration()
+        self.finish_migration()
+
+
+def split_initial(layout, pos, vel):
+    """Host-side initial distribution: per rank, the (pos, vel) rows it owns, in ascending index order."""
+    own = layout.owner(np.asarray(pos)[:, layout.axis])
+    return [(np.ascontiguousarray(pos[own == r]), np.ascontiguousarray(vel[own == r])) for r in range(layout.world)]
+
+
+def run_loopback(sims, steps):
+    """Single-process emulation: all ranks post, then all ranks collect, phase by phase."""
+    for _ in range(steps):
+        for s in sims:
+            s.post_halo()
+        for s in sims:
+            s.step_with_halo()
+        for s in sims:
+            s.post_migration()
+        for s in sims:
+            s.finish_migration()

@@ -1,0 +1,52 @@
+"""Test-only backend for paper_2311_15088_b200.slab: selection in numpy, the step on the CPU oracle (CPU tensors).
+
+It lets the decomposition logic (who owns what, what travels as a ghost, who migrates) be exercised end to end on the
+CPU -- under torch.distributed / gloo with one process per rank -- against the undecomposed oracle step."""
+import numpy as np
+import torch
+
+from oracle import refbind as R
+
+
+class OracleBackend:
+    def __init__(self, sph):
+        self.sph = sph
+
+    def to_device(self, a):
+        return torch.from_numpy(np.ascontiguousarray(a, np.float32).copy())
+
+    def pack(self, pos, vel, n, axis, lo, hi):
+        x = pos[:n, axis].numpy()
+        sel = torch.from_numpy((x >= np.float32(lo)) & (x < np.float32(hi)))
+        return pos[:n][sel].clone(), vel[:n][sel].clone()
+
+    def step(self, pos, vel):
+        out = R.step(self.sph, pos.numpy(), vel.numpy())
+        pos.copy_(torch.from_numpy(out["pos"]))
+        vel.copy_(torch.from_numpy(out["vel"]))
+
+    def cat(self, parts):
+        return torch.cat(parts, 0) if len(parts) > 1 else parts[0].clone()
+
+    def close(self):
+        pass
+
+
+def tagged_state(cfg, seed=5, speed=6.0):
+    """Config state with the particle id in pos.w (carried through by the step) and velocities that make particles
+    cross slab faces within a few steps."""
+    from paper_2311_15088_b200 import workloads as W
+    pos = cfg["pos"].copy()
+    pos[:, 3] = np.arange(cfg["n"], dtype=np.float32)
+    vel = W.uniform_box(cfg["n"], (-speed,) * 3, (speed,) * 3, seed, 30)
+    return pos, vel
+
+
+def gather_by_id(parts, n):
+    """parts: list of (pos, vel) numpy arrays of the ranks -> (pos, vel) in id order; checks ids are a permutation."""
+    pos = np.concatenate([p for p, _ in parts], 0)
+    vel = np.concatenate([v for _, v in parts], 0)
+    ids = pos[:, 3].astype(np.int64)
+    assert ids.shape[0] == n and np.array_equal(np.sort(ids), np.arange(n)), "particles lost or duplicated"
+    order = np.argsort(ids)
+    return pos[order], vel[order]

@@ -1,0 +1,109 @@
+"""N2 host logic on the CPU: slab layout, and the decomposed step end to end under gloo with world_size 2 (one process
+per rank, neighbour exchange through torch.distributed) against the undecomposed oracle step."""
+import os
+import subprocess
+import sys
+
+import numpy as np
+
+from paper_2311_15088_b200 import slab as S
+from paper_2311_15088_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_slab_layout_owns_every_coordinate_once():
+    sph = W.config(3, scale=4)["sph"]  # box [0,2] x [0,1] x [0,1], h = 1/32: 64 cells along x
+    for world in (1, 2, 3, 5):
+        lay = S.SlabLayout(sph, world)
+        assert lay.axis == 0 and lay.dim == 64 and len(lay.faces) == world - 1
+        b = [lay.bounds(r) for r in range(world)]
+        assert b[0][0] == -np.inf and b[-1][1] == np.inf
+        for r in range(world - 1):
+            assert b[r][1] == b[r + 1][0]  # faces shared, slabs contiguous
+            assert abs(b[r][1] / sph["h"] - round(b[r][1] / sph["h"])) < 1e-6  # on a cell boundary
+        x = np.float32(np.linspace(-0.5, 2.5, 1001))
+        own = lay.owner(x)
+        for r in range(world):
+            lo, hi = b[r]
+            assert np.array_equal(own == r, (x >= np.float32(lo)) & (x < np.float32(hi)))
+
+
+def test_loopback_decomposition_equals_undecomposed_oracle():
+    # 3 emulated ranks in one process, oracle as the stepper: four steps with migration; every particle ends where the
+    # undecomposed oracle puts it (the neighbour sets are identical; only the order of the binary64 sums can differ)
+    from oracle import refbind as R
+    from tests.slabutil import OracleBackend, gather_by_id, tagged_state
+    cfg = W.config(1)
+    pos, vel = tagged_state(cfg)
+    lay = S.SlabLayout(cfg["sph"], 3)
+    ex = S.LoopbackExchange(3)
+    be = OracleBackend(cfg["sph"])
+    sims = [S.SlabSim(lay, r, be, ex, be.to_device(p), be.to_device(v)) for r, (p, v) in enumerate(S.split_initial(lay, pos, vel))]
+    rp, rv = pos, vel
+    moved = 0
+    for _ in range(4):
+        S.run_loopback(sims, 1)
+        out = R.step(cfg["sph"], rp, rv)
+        rp, rv = out["pos"], out["vel"]
+        moved += sum(s.stats["migrated_out"] for s in sims)
+        for s in sims:  # every rank owns exactly the particles of its slab
+            x = s.pos[:, lay.axis].numpy()
+            assert ((x >= np.float32(s.lo)) & (x < np.float32(s.hi))).all()
+    assert moved > 0 and sims[0].stats["ghosts"] > 0 and sims[1].stats["ghosts"] > 0  # (rank 2's slab is empty)
+    gp, gv = gather_by_id([(s.pos.numpy(), s.vel.numpy()) for s in sims], cfg["n"])
+    assert np.abs(gp[:, :3] - rp[:, :3]).max() <= 1e-6 and np.abs(gv[:, :3] - rv[:, :3]).max() <= 1e-5
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import numpy as np, torch
+import torch.distributed as dist
+from paper_2311_15088_b200 import slab as S, workloads as W
+from tests.slabutil import OracleBackend, tagged_state
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)
+cfg = W.config(1)
+pos, vel = tagged_state(cfg)
+lay = S.SlabLayout(cfg["sph"], world)
+be = OracleBackend(cfg["sph"])
+p, v = S.split_initial(lay, pos, vel)[rank]
+sim = S.SlabSim(lay, rank, be, S.DistExchange(dist, rank, world, torch.device("cpu")), be.to_device(p), be.to_device(v))
+for _ in range(3):
+    sim.step()
+np.save({out!r} % rank, np.concatenate([sim.pos.numpy(), sim.vel.numpy()], 1))
+dist.barrier()
+dist.destroy_process_group()
+print("rank", rank, "ok", sim.n_owned, sim.stats)
+"""
+
+
+def test_decomposed_step_under_gloo_world_size_2(tmp_path):
+    from oracle import refbind as R
+    from tests.slabutil import gather_by_id, tagged_state
+    script = tmp_path / "worker.py"
+    out_pat = str(tmp_path / "rank%d.npy")
+    script.write_text(_WORKER.format(root=ROOT, out=out_pat))
+    port = 29900 + os.getpid() % 90
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), CUDA_VISIBLE_DEVICES="", OMP_NUM_THREADS="2")
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    for rank, p in enumerate(procs):
+        out, _ = p.communicate(timeout=300)
+        assert p.returncode == 0, out
+        assert "rank %d ok" % rank in out
+    cfg = W.config(1)
+    rp, rv = tagged_state(cfg)
+    for _ in range(3):
+        o = R.step(cfg["sph"], rp, rv)
+        rp, rv = o["pos"], o["vel"]
+    parts = []
+    for rank in range(2):
+        a = np.load(out_pat % rank)
+        parts.append((a[:, :4], a[:, 4:]))
+    gp, gv = gather_by_id(parts, cfg["n"])
+    assert np.abs(gp[:, :3] - rp[:, :3]).max() <= 1e-6 and np.abs(gv[:, :3] - rv[:, :3]).max() <= 1e-5
