@@ -28,6 +28,11 @@
  *   voxel SDF ................................ pinned (one particle: phi = |x-x1| - rbar; symmetric pair)
  *   MC table ................................. pinned (P:542 worked example edge_table[8]=0x80c, crack-free
  *                                                      faces, edge cover, orientation)
+ *   indexed mesh (N3) ........................ welding pinned (expands to the triangle soup bitwise, Euler characteristic
+ *                                              on the index buffer); the NORMAL formula is ours (D:A-NORMAL): invariants
+ *                                              only (exact on a plane, radial on a sphere): PARITY UNPINNED
+ *   obstacle avoidance (N4) .................. invariants only (hand-evaluated single cell, zero grid, range walk = all
+ *                                              cells, sphere pushes outwards); the rule is ours (D:C-OBST): PARITY UNPINNED
  *   MC end to end ............................ pinned (analytic sphere: closed, Euler char 2, area, volume)
  */
 #ifndef ORACLE_REF_H
