@@ -22,7 +22,7 @@ def _polygonise_gpu(sim, mp, phi_np, capacity):
     return tris.cpu().numpy()[:min(nt, capacity)], nt
 
 
-@pytest.mark.parametrize("idx,scale", [(1, None), (2, None), (3, 2), (4, 4)])
+@pytest.mark.parametrize("idx,scale", [(1, None), (2, None), (3, 2), (4, 4), (5, 4)])
 def test_sdf_and_polygonise_on_configs(idx, scale):
     cfg = W.config(idx, scale=scale)
     mp = W.mc_params(cfg)
