@@ -281,7 +281,8 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
       cudaMalloc(&ctx->nbr.list, (size_t)nbr_rows() * (ctx->nbr.stride = (uint32_t)((nn + 63) & ~(size_t)63)) * 2) != cudaSuccess ||
       cudaMalloc(&ctx->sdf_first, (size_t)(ctx->sdf_first_cap = (uint32_t)(sc.grid.dim[0] + sc.grid.dim[1] +
                                                                           sc.grid.dim[2] + 3 * (2 * 16 + 3))) * 4) !=
-          cudaSuccess || cudaMalloc(&ctx->scan.ticket, 4) != cudaSuccess)
+          cudaSuccess || cudaMalloc(&ctx->scan.ticket, 4) != cudaSuccess ||
+      cudaMalloc(&ctx->scan.ctl, 8) != cudaSuccess)
     return bail(SPH_E_CUDA);
   ctx->max_tiles = std::max(std::max(grid_scan_tiles(sc.grid.C), grid_scan_tiles(ctx->boid_cells_cap)),
                             std::max(std::max(mc_num_tiles((uint32_t)G), mc_word_tiles((uint32_t)G)), 1u));
@@ -290,17 +291,21 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   cudaMemset(ctx->scan.ticket, 0, 4);
   {
     const size_t mt = std::max(std::max(mc_num_tiles((uint32_t)G), mc_word_tiles((uint32_t)G)), 1u);
-    if (cudaMalloc(&ctx->scan_mc.status, mt * 8) != cudaSuccess || cudaMalloc(&ctx->scan_mc.ticket, 4) != cudaSuccess)
+    if (cudaMalloc(&ctx->scan_mc.status, mt * 8) != cudaSuccess || cudaMalloc(&ctx->scan_mc.ticket, 4) != cudaSuccess ||
+        cudaMalloc(&ctx->scan_mc.ctl, 8) != cudaSuccess)
       return bail(SPH_E_CUDA);
     cudaMemset(ctx->scan_mc.status, 0, mt * 8);
     cudaMemset(ctx->scan_mc.ticket, 0, 4);
-    ctx->scan_mc.ticket_base = 0;
+    {
+      const uint32_t ctl0[2] = {1u, 0u};  // epoch 1: status words of zeros read as "not ready"
+      cudaMemcpy(ctx->scan_mc.ctl, ctl0, 8, cudaMemcpyHostToDevice);
+      cudaMemcpy(ctx->scan.ctl, ctl0, 8, cudaMemcpyHostToDevice);
+    }
     ctx->scan_mc.epoch = 0;
   }
   cudaMemset(ctx->n_tris_dev, 0, 4);
   cudaMemset(ctx->mc_nwork, 0, 8);
   cudaMemset(ctx->mc_bits, 0, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4);
-  ctx->scan.ticket_base = 0;
   ctx->scan.epoch = 0;
   if (cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
       cudaStreamCreateWithFlags(&ctx->surf, cudaStreamNonBlocking) != cudaSuccess ||
@@ -322,7 +327,7 @@ int sph_destroy(sph_ctx* ctx) {
   free_grid(ctx->pg);
   free_grid(ctx->bg);
   cudaFree(ctx->nbr.list), cudaFree(ctx->nbr.cnt), cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->n_verts_dev), cudaFree(ctx->mc_prefix), cudaFree(ctx->mc_work), cudaFree(ctx->mc_nwork), cudaFree(ctx->sdf_first);
-  cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket), cudaFree(ctx->scan_mc.status), cudaFree(ctx->scan_mc.ticket);
+  cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket), cudaFree(ctx->scan_mc.status), cudaFree(ctx->scan_mc.ticket), cudaFree(ctx->scan.ctl), cudaFree(ctx->scan_mc.ctl);
   sph_profile_enable(ctx, 0);
   free(ctx->prof.recs);
   if (ctx->side) cudaStreamDestroy(ctx->side);

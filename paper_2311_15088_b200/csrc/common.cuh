@@ -53,14 +53,15 @@ __device__ __forceinline__ double warp_sum_f64(double v) {
 // ---- single-pass device-wide exclusive scan: block-local scan + decoupled look-back -------------------
 // One 64-bit status word per tile: high 32 bits = flag, low 32 bits = value.  Flags are tagged with the
 // launch epoch (2*epoch+1 = tile aggregate ready, 2*epoch+2 = inclusive prefix ready), so words left by an
-// earlier launch read as "not ready" and the array never needs clearing.  Tiles are handed out by a
-// monotonically increasing ticket counter (base passed by the host), so a tile's predecessors are always
-// already running: the spin below cannot deadlock.
+// earlier launch read as "not ready" and the array never needs clearing.  Tiles are handed out by a ticket
+// counter, so a tile's predecessors are always already running: the spin below cannot deadlock.  Epoch and ticket
+// live in device memory and are advanced / reset by the last block of a launch to retire (scan_end), so a launch
+// carries no host-side state and the kernels can be replayed from a CUDA graph.
 struct ScanState {
   unsigned long long* status;  // [max_tiles]
-  uint32_t* ticket;            // monotonically increasing across launches
-  uint32_t ticket_base;        // value of *ticket when this launch starts
-  uint32_t epoch;              // launch counter, > 0
+  uint32_t* ticket;            // next tile of the running launch; back to 0 when the launch's last block retires
+  uint32_t* ctl;               // [2] = {launch epoch (> 0), blocks of the running launch that have retired}
+  uint32_t epoch;              // the running launch's epoch: filled in on the device by scan_begin (0 on the host)
 };
 
 __device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
@@ -104,6 +105,26 @@ __device__ __forceinline__ uint32_t lookback_exclusive(const ScanState& st, uint
   }
   if (lane == 0) st_status(st.status + tile, flagP | (exclusive + aggregate));
   return exclusive;
+}
+
+// Thread 0 of a block: take a tile and read the launch's epoch (unchanged until every block has retired).
+__device__ __forceinline__ uint32_t scan_begin(const ScanState& st, uint32_t* epoch_out) {
+  const uint32_t tile = atomicAdd(st.ticket, 1u);
+  uint32_t e;
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(e) : "l"(st.ctl) : "memory");
+  *epoch_out = e;
+  return tile;
+}
+// Thread 0 of a block, once the block no longer reads or writes the status words: the last of the launch's n_tiles
+// blocks re-arms the state for the next launch.
+__device__ __forceinline__ void scan_end(const ScanState& st, uint32_t n_tiles) {
+  __threadfence();
+  if (atomicAdd(st.ctl + 1, 1u) == n_tiles - 1u) {
+    *st.ticket = 0u;
+    st.ctl[1] = 0u;
+    st.ctl[0] = st.epoch + 1u;
+    __threadfence();
+  }
 }
 
 // Block-wide exclusive scan of one value per thread (blockDim.x <= 1024, multiple of 32).

@@ -13,7 +13,10 @@ constexpr int kScanTile = kThreads * kScanItems;  // 2048 cells per tile
 // S1 + S2 (P:426-432 set_particle_count): key = hash(get_cell(p)); rank = atomicAdd(count[key], 1).
 __global__ void __launch_bounds__(kThreads) k_hash_count(GridDesc g, const float4* __restrict__ pos, uint32_t n,
                                                          uint32_t* __restrict__ key, uint32_t* __restrict__ rank,
-                                                         uint32_t* __restrict__ count, uint32_t* __restrict__ box_part) {
+                                                         uint32_t* __restrict__ count, uint32_t* __restrict__ box_part,
+                                                         uint32_t* __restrict__ aabb) {
+  // the bounding box of this build starts empty (the scan kernel, which runs next, folds the partials into it)
+  if (blockIdx.x == 0 && threadIdx.x < 6) aabb[threadIdx.x] = threadIdx.x < 3 ? 0xffffffffu : 0u;
   const uint32_t i = blockIdx.x * kThreads + threadIdx.x;
   const bool in = i < n;
   const float4 p = __ldg(pos + (in ? i : n - 1));
@@ -60,9 +63,9 @@ __global__ void __launch_bounds__(kThreads) k_hash_count(GridDesc g, const float
 __global__ void __launch_bounds__(kThreads) k_scan_cells(uint32_t* __restrict__ count, uint32_t* __restrict__ start,
                                                          uint32_t C, ScanState st,
                                                          const uint32_t* __restrict__ box_part, uint32_t n_parts,
-                                                         uint32_t* __restrict__ aabb, uint32_t* __restrict__ aabb_next) {
+                                                         uint32_t* __restrict__ aabb) {
   __shared__ uint32_t s_scan[33];
-  if (blockIdx.x == 0 && threadIdx.x < 6) aabb_next[threadIdx.x] = threadIdx.x < 3 ? 0xffffffffu : 0u;  // empty box
+  if (n_parts == 0 && blockIdx.x == 0 && threadIdx.x < 6) aabb[threadIdx.x] = threadIdx.x < 3 ? 0xffffffffu : 0u;  // no points
   if (threadIdx.x >= 32 && threadIdx.x < 64) {  // warp 1 folds this block's share of the bounding-box partials
     const uint32_t lane = threadIdx.x - 32;
     uint32_t v[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
@@ -88,10 +91,11 @@ __global__ void __launch_bounds__(kThreads) k_scan_cells(uint32_t* __restrict__ 
       }
     }
   }
-  __shared__ uint32_t s_tile, s_base;
-  if (threadIdx.x == 0) s_tile = atomicAdd(st.ticket, 1u) - st.ticket_base;
+  __shared__ uint32_t s_tile, s_base, s_epoch;
+  if (threadIdx.x == 0) s_tile = scan_begin(st, &s_epoch);
   __syncthreads();
   const uint32_t tile = s_tile;
+  st.epoch = s_epoch;
   const uint32_t first = tile * kScanTile + threadIdx.x * kScanItems;
   const bool full = first + kScanItems <= C;
   uint32_t v[kScanItems];
@@ -118,7 +122,10 @@ __global__ void __launch_bounds__(kThreads) k_scan_cells(uint32_t* __restrict__ 
   uint32_t excl = block_exclusive_scan(sum, s_scan, &total);
   if (threadIdx.x < 32) {
     const uint32_t base = lookback_exclusive(st, tile, total);
-    if (threadIdx.x == 0) s_base = base;
+    if (threadIdx.x == 0) {
+      s_base = base;
+      scan_end(st, gridDim.x);
+    }
   }
   __syncthreads();
   excl += s_base;
@@ -278,17 +285,13 @@ void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const f
   const int k0 = boid_grid ? K_BOID_HASH_COUNT : K_HASH_COUNT;
   if (n > 0) {
     prof->begin(k0 + 0, s);
-    k_hash_count<<<blocks, kThreads, 0, s>>>(g, pos, n, b.key, b.rank, b.count, b.box_part);
+    k_hash_count<<<blocks, kThreads, 0, s>>>(g, pos, n, b.key, b.rank, b.count, b.box_part, b.aabb);
     prof->end(s);
   }
   const uint32_t tiles = grid_scan_tiles(g.C);
-  scan.epoch += 1;
   prof->begin(k0 + 1, s);
-  // the scan also empties the OTHER bounding-box slot, which the next build fills
-  k_scan_cells<<<tiles, kThreads, 0, s>>>(b.count, b.start, g.C, scan, b.box_part, n > 0 ? blocks : 0u,
-                                          b.aabb + 6 * b.slot, b.aabb + 6 * (b.slot ^ 1));
+  k_scan_cells<<<tiles, kThreads, 0, s>>>(b.count, b.start, g.C, scan, b.box_part, n > 0 ? blocks : 0u, b.aabb);
   prof->end(s);
-  scan.ticket_base += tiles;
   if (n > 0) {
     prof->begin(k0 + 2, s);
     k_scatter<<<blocks, kThreads, 0, s>>>(b.key, b.rank, b.start, n, b.slot_id);
@@ -297,8 +300,7 @@ void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const f
     k_reorder<<<blocks, kThreads, 0, s>>>(b.key, b.start, b.slot_id, pos, vel, n, b.perm, b.posS, b.velS);
     prof->end(s);
   }
-  b.aabb_now = b.aabb + 6 * b.slot;
-  b.slot ^= 1;
+  b.aabb_now = b.aabb;
 }
 
 void launch_hashgrid_count(const GridDesc& g, float h2, const float4* pos, uint32_t n, uint32_t cap, uint32_t* tracker,
