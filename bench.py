@@ -305,6 +305,23 @@ def main():
         ev[2 * k + 2].record()
     torch.cuda.synchronize()
     t_serial = ev[0].elapsed_time(ev[2 * K]) * 1e-3
+    # (3) CUDA graphs: the synchronous frame captured once and replayed K times (one launch per frame), and four
+    #     pipelined frames per graph (inside it the surface pass of a frame runs beside the next frame's SPH step)
+    def time_graph(frames, pipelined):
+        fr.capture(frames=frames, pipelined=pipelined)
+        reps = max(1, (K + frames - 1) // frames)
+        evg = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ranks.barrier()
+        torch.cuda.synchronize()
+        evg[0].record()
+        for _ in range(reps):
+            fr.replay()
+        evg[1].record()
+        torch.cuda.synchronize()
+        return evg[0].elapsed_time(evg[1]) * 1e-3 * K / (reps * frames)  # scaled to K frames
+
+    t_graph = time_graph(1, False)
+    t_graph4 = time_graph(4, True)
     t_sim = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(K)) * 1e-3
     t_mc = sum(ev[2 * k + 1].elapsed_time(ev[2 * k + 2]) for k in range(K)) * 1e-3
     # ---- per-kernel durations: the same K frames again with a CUDA event pair around every launch (the pairs cost a
@@ -369,12 +386,16 @@ def main():
     for a in range(3):
         cb *= max(1, math.ceil((bpar["space_max"][a] - bpar["space_min"][a]) / cell_b))
 
-    # both loops ran the same K frames; `value` is the faster way to run them (the overlap pays when the working set
-    # fits L2, config 4, and costs when the two passes evict each other, config 5); both times are reported
+    # all three loops ran the same K frames; `value` is the fastest way to run them (the overlap pays when the working
+    # set fits L2, config 4, and costs when the two passes evict each other, config 5; the graph pays when the frame is
+    # launch-bound, configs 1-3); all three times are reported
     t_pipe_max, units = ranks.combine(t_total, n * K)
     t_serial_max, _ = ranks.combine(t_serial, 0.0)
-    pipelined = t_pipe_max <= t_serial_max
-    t_max = min(t_pipe_max, t_serial_max)
+    t_graph_max, _ = ranks.combine(t_graph, 0.0)
+    t_graph4_max, _ = ranks.combine(t_graph4, 0.0)
+    t_max = min(t_pipe_max, t_serial_max, t_graph_max, t_graph4_max)
+    mode = {t_pipe_max: "pipelined", t_serial_max: "synchronous", t_graph_max: "graph",
+            t_graph4_max: "graph of 4 pipelined frames"}[t_max]
     t_sim_max, t_mc_max = ranks.reduce_max([t_sim, t_mc])
     value = units / t_max
     world = ranks.world
@@ -453,13 +474,15 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": "particle-updates/s", "n_gpus": world, "steps": K,
             "warmup": args.warmup, "ms_per_step": 1e3 * t_max / K, "ms_per_step_pipelined": 1e3 * t_pipe_max / K,
-            "ms_per_step_serial": 1e3 * t_serial_max / K, "higher_is_better": True, "scaling": "weak",
+            "ms_per_step_serial": 1e3 * t_serial_max / K, "ms_per_step_graph": 1e3 * t_graph_max / K,
+            "ms_per_step_graph_pipelined4": 1e3 * t_graph4_max / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": cfg["name"], "particles": n, "boids": nb, "mc_points_per_axis": G,
                        "grid_cells": C, "triangles_last_frame": n_tris, "parallelism": "replicas x%d" % world,
-                       "pipelining": ("on" if pipelined else "off") + ": both loops are timed over the same K frames -- the "
-                                     "surface pass of frame t beside the SPH step of frame t+1 (mc_extract_async), and the "
-                                     "synchronous calls -- `value` is the faster one; `parts` come from the synchronous loop",
+                       "frame_loop": mode + ": the same K frames are timed four ways -- the surface pass of frame t beside "
+                                     "the SPH step of frame t+1 (mc_extract_async), the synchronous calls, the synchronous frame "
+                                     "replayed from a CUDA graph, and a CUDA graph of four pipelined frames -- `value` is the "
+                                     "fastest; `parts` come from the synchronous loop",
                        "l2": "no explicit flush: the frame's working set (%.0f MB) exceeds the %.0f MB L2 and "
                              "the state changes every step" % (state_bytes / 1e6, L2_BYTES / 1e6)},
             "parts": {

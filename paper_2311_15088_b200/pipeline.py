@@ -70,6 +70,32 @@ class Frame:
             self.n_tris = nt
         return nt
 
+    def capture(self, frames=1, pipelined=False):
+        """Capture `frames` whole frames into a CUDA graph; replay() then runs them with one launch.  The library keeps
+        no per-launch state on the host (scan epochs, work counters and the bounding box live in device memory), and
+        the state of the context after a frame equals the state before it, so the captured sequence is valid for
+        every later frame.  pipelined: inside the graph the surface pass of a frame is forked (mc_extract_async) and
+        runs beside the next frame's SPH step; the last one is joined before the graph ends.  The frame just before
+        the capture runs eagerly."""
+        torch = self.torch
+        self.frame()
+        torch.cuda.synchronize()
+        self.graph = torch.cuda.CUDAGraph()
+        self.graph_frames = frames
+        with torch.cuda.graph(self.graph):
+            for _ in range(frames):
+                self.sim()
+                if pipelined:
+                    self.surface_async()
+                else:
+                    self.surface()
+            if pipelined:
+                self.wait()
+        return self.graph
+
+    def replay(self):
+        self.graph.replay()
+
     def frame(self, sync=False):
         self.sim()
         if self.with_mc:

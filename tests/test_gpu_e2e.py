@@ -81,3 +81,47 @@ def test_async_surface_pass_is_bitwise_the_synchronous_one():
             assert np.array_equal(states[t].cpu().numpy(), pos)
         with pytest.raises(B.SphError):
             B.mc_wait(fb.ctx)  # nothing pending any more
+
+
+def test_cuda_graph_replay_is_bitwise_the_eager_frame():
+    # a frame captured once into a CUDA graph and replayed: state and mesh identical, bit for bit, to eager frames
+    # (the library keeps no per-launch host state: scan epochs, work counters and the bounding box live on the device)
+    from paper_2311_15088_b200.pipeline import Frame
+    cfg = W.config(2, scale=2)
+    eager = []
+    with Frame(cfg) as fa:
+        for _ in range(5):
+            fa.sim()
+            nt = fa.surface(sync=True)
+            eager.append((nt, fa.tris[:nt].cpu().numpy().copy(), fa.pos.cpu().numpy().copy(), fa.bpos.cpu().numpy().copy()))
+    with Frame(cfg) as fb:
+        fb.capture()  # runs frame 1 eagerly, then captures (the capture itself does not execute)
+        for t in range(1, 5):
+            fb.replay()
+            torch.cuda.synchronize()
+            nt = int(B.mc_extract(fb.ctx, fb.mc, torch.zeros_like(fb.tris)))  # count of the same state, eagerly
+            want_nt, want_tris, want_pos, want_bpos = eager[t]
+            assert nt == want_nt
+            assert np.array_equal(fb.tris[:nt].cpu().numpy(), want_tris)
+            assert np.array_equal(fb.pos.cpu().numpy(), want_pos) and np.array_equal(fb.bpos.cpu().numpy(), want_bpos)
+
+
+def test_cuda_graph_of_pipelined_frames_matches_eager():
+    # three frames per graph, inside it every surface pass forked beside the next frame's SPH step: after each replay
+    # the state and the mesh are those of the eager frames 3, 6, ... (frame 1 runs eagerly before the capture... so 4, 7)
+    from paper_2311_15088_b200.pipeline import Frame
+    cfg = W.config(2, scale=2)
+    eager = []
+    with Frame(cfg) as fa:
+        for _ in range(7):
+            fa.sim()
+            nt = fa.surface(sync=True)
+            eager.append((nt, fa.tris[:nt].cpu().numpy().copy(), fa.pos.cpu().numpy().copy()))
+    with Frame(cfg) as fb:
+        fb.capture(frames=3, pipelined=True)  # eager frame 1, then frames 2-4 per replay
+        for rep in range(2):
+            fb.replay()
+            torch.cuda.synchronize()
+            want_nt, want_tris, want_pos = eager[3 * (rep + 1)]
+            assert np.array_equal(fb.pos.cpu().numpy(), want_pos)
+            assert np.array_equal(fb.tris[:want_nt].cpu().numpy(), want_tris)
