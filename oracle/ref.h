@@ -31,6 +31,8 @@
  *   indexed mesh (N3) ........................ welding pinned (expands to the triangle soup bitwise, Euler characteristic
  *                                              on the index buffer); the NORMAL formula is ours (D:A-NORMAL): invariants
  *                                              only (exact on a plane, radial on a sphere): PARITY UNPINNED
+ *   mesh connectivity (N3) ................... pinned (scipy.sparse.csgraph.connected_components on random triangle sets,
+ *                                              k separated spheres -> k equal components, hand-made chains)
  *   obstacle avoidance (N4) .................. invariants only (hand-evaluated single cell, zero grid, range walk = all
  *                                              cells, sphere pushes outwards); the rule is ours (D:C-OBST): PARITY UNPINNED
  *   MC end to end ............................ pinned (analytic sphere: closed, Euler char 2, area, volume)
@@ -129,6 +131,13 @@ int ref_mc_polygonise(const ref_mc_params* mp, const float* phi, float* tris, ui
  * nothing past a capacity is written.  Returns 1 if a capacity was too small. */
 int ref_mc_indexed(const ref_mc_params* mp, const float* phi, float* verts, float* normals, uint32_t vert_capacity,
                    uint32_t* indices, uint32_t tri_capacity, uint32_t* n_verts, uint32_t* n_tris);
+
+/* N3 connectivity (Table 2; D:A-CONNECT): connected components of an indexed mesh, two triangles
+ * being connected when they share a vertex.  label[n_verts] (may be NULL) = smallest vertex id of the vertex's
+ * component; n_components counts every vertex's component (an unused vertex is one, with no triangle);
+ * largest_tris = triangles of the component that has most.  Returns -1 if an index is out of range. */
+int ref_mesh_components(const uint32_t* indices, uint32_t n_tris, uint32_t n_verts, uint32_t* label,
+                        uint32_t* n_components, uint32_t* largest_tris);
 
 /* The generated table (D:M-TABLE): tri[256][16] edge ids terminated by -1, ntri[256], edge_table[256]. */
 void ref_mc_table(int8_t* tri, uint8_t* ntri, uint16_t* edge_table);

@@ -339,4 +339,57 @@ int ref_mc_indexed(const ref_mc_params* mp, const float* phi, float* verts, floa
   return (nv > vert_capacity || count > tri_capacity) ? 1 : 0;
 }
 
+// N3, connectivity ("for the triangles to connect with each other", Table 2 last column P:595-602; reading
+// D:A-CONNECT): triangles are connected when they share a welded vertex; a component is a maximal connected set.
+// label[v] = the smallest vertex id of v's component; a vertex no triangle uses is a component of its own with no
+// triangle.  Plain flood fill over the vertex -> triangle incidence lists, components discovered in ascending
+// vertex id, so the seed of each fill is the component's smallest id.
+int ref_mesh_components(const uint32_t* indices, uint32_t n_tris, uint32_t n_verts, uint32_t* label,
+                        uint32_t* n_components, uint32_t* largest_tris) {
+  if (n_components) *n_components = 0;
+  if (largest_tris) *largest_tris = 0;
+  for (uint64_t e = 0; e < 3ull * n_tris; ++e)
+    if (indices[e] >= n_verts) return -1;
+  std::vector<uint32_t> first(n_verts + 1ull, 0), inc(3ull * n_tris);
+  for (uint64_t e = 0; e < 3ull * n_tris; ++e) ++first[indices[e] + 1ull];
+  for (uint32_t v = 0; v < n_verts; ++v) first[v + 1ull] += first[v];
+  std::vector<uint32_t> fill(first.begin(), first.end() - 1);
+  for (uint32_t t = 0; t < n_tris; ++t)
+    for (int c = 0; c < 3; ++c) inc[fill[indices[3ull * t + c]]++] = t;
+  std::vector<uint32_t> lab(n_verts, 0xffffffffu), stack;
+  std::vector<char> seen_tri(n_tris, 0);
+  uint32_t comps = 0, largest = 0;
+  for (uint32_t seed = 0; seed < n_verts; ++seed) {
+    if (lab[seed] != 0xffffffffu) continue;
+    ++comps;
+    uint32_t tris_here = 0;
+    lab[seed] = seed;
+    stack.assign(1, seed);
+    while (!stack.empty()) {
+      const uint32_t v = stack.back();
+      stack.pop_back();
+      for (uint32_t q = first[v]; q < first[v + 1ull]; ++q) {
+        const uint32_t t = inc[q];
+        if (seen_tri[t]) continue;
+        seen_tri[t] = 1;
+        ++tris_here;
+        for (int c = 0; c < 3; ++c) {
+          const uint32_t w = indices[3ull * t + c];
+          if (lab[w] == 0xffffffffu) {
+            lab[w] = seed;
+            stack.push_back(w);
+          }
+        }
+      }
+    }
+    if (tris_here > largest) largest = tris_here;
+  }
+  if (label)
+    for (uint32_t v = 0; v < n_verts; ++v) label[v] = lab[v];
+  if (n_components) *n_components = comps;
+  if (largest_tris) *largest_tris = largest;
+  return 0;
+}
+
+
 }  // extern "C"

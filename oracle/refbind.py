@@ -65,6 +65,7 @@ def lib():
         L.ref_voxel_sdf.argtypes = [vp, vp, vp, _u32, C.c_int, vp]
         L.ref_mc_polygonise.argtypes = [vp, vp, vp, _u32, vp, vp]
         L.ref_mc_indexed.argtypes = [vp, vp, vp, vp, _u32, vp, _u32, vp, vp]
+        L.ref_mesh_components.argtypes = [vp, _u32, _u32, vp, vp, vp]
         L.ref_mc_table.argtypes = [vp, vp, vp]
         L.ref_mc_table.restype = None
         L.ref_mc_numbering.argtypes = [vp, vp]
@@ -220,6 +221,17 @@ def mc_indexed(mp, phi):
                               C.byref(nt))
     assert rc == 0
     return verts[:nv.value], normals[:nv.value], idx[:nt.value]
+
+
+def mesh_components(indices, n_verts):
+    """N3 connectivity: returns (label (V,) uint32 = smallest vertex id of the component, n_components, largest_tris)."""
+    idx = np.ascontiguousarray(indices, np.uint32).reshape(-1, 3)
+    label = np.zeros(max(int(n_verts), 1), np.uint32)
+    nc, big = _u32(0), _u32(0)
+    rc = lib().ref_mesh_components(_p(idx) if idx.size else None, idx.shape[0], int(n_verts), _p(label), C.byref(nc),
+                                   C.byref(big))
+    assert rc == 0
+    return label[:int(n_verts)], int(nc.value), int(big.value)
 
 
 def mc_table():

@@ -236,3 +236,60 @@ def test_indexed_plane_normals_are_exact_and_border_is_one_sided():
     # flipped sign: fluid above the plane, normals point down
     v2, n2, _ = R.mc_indexed(mp, -phi)
     assert np.array_equal(v2, verts) and np.abs(n2 - np.array([0, 0, -1], np.float32)).max() < 1e-6
+
+
+# ---- N3 connectivity (Table 2 last column; reading D:A-CONNECT) -----------------------------------------------
+def test_mesh_components_match_scipy_on_random_triangle_sets():
+    # a library routine as the pin: components of the graph with an edge between the vertices of every triangle
+    from scipy.sparse import coo_matrix
+    from scipy.sparse.csgraph import connected_components
+    rng = np.random.default_rng(11)
+    for V, T in ((1, 0), (7, 0), (3, 1), (40, 9), (300, 120), (5000, 1700), (5000, 9000)):
+        idx = rng.integers(0, V, size=(T, 3)).astype(np.uint32)  # degenerate triangles (repeated ids) included
+        label, nc, big = R.mesh_components(idx, V)
+        i = idx.astype(np.int64)
+        rows = np.concatenate([i[:, 0], i[:, 0]]) if T else np.zeros(0, np.int64)
+        cols = np.concatenate([i[:, 1], i[:, 2]]) if T else np.zeros(0, np.int64)
+        g = coo_matrix((np.ones(rows.size), (rows, cols)), shape=(V, V))
+        n_ref, lab_ref = connected_components(g, directed=False)
+        assert nc == n_ref
+        # same partition, and the label is the smallest vertex id of the part
+        smallest = np.full(n_ref, V, np.int64)
+        np.minimum.at(smallest, lab_ref, np.arange(V))
+        assert np.array_equal(label.astype(np.int64), smallest[lab_ref])
+        per = np.bincount(lab_ref[i[:, 0]], minlength=n_ref) if T else np.zeros(1, np.int64)
+        assert big == per.max()
+
+
+def test_mesh_components_hand_made_chain_and_vertex_only_contact():
+    # a strip of triangles sharing edges, one triangle touching it in a single vertex (connected, D:A-CONNECT),
+    # one apart, one unused vertex
+    idx = np.array([[0, 1, 2], [1, 2, 3], [2, 3, 4], [4, 5, 6], [8, 9, 10]], np.uint32)
+    label, nc, big = R.mesh_components(idx, 11)
+    assert label.tolist() == [0, 0, 0, 0, 0, 0, 0, 7, 8, 8, 8]
+    assert nc == 3 and big == 4
+    # relabelling the vertices changes the labels, not the partition sizes
+    perm = np.random.default_rng(0).permutation(11).astype(np.uint32)
+    _, nc2, big2 = R.mesh_components(perm[idx], 11)
+    assert (nc2, big2) == (3, 4)
+
+
+def test_mesh_components_of_separated_spheres():
+    # k spheres further apart than a cube: k closed components with the triangle counts of the spheres extracted one
+    # by one; one sphere: a single component holding 100 % of the triangles
+    G = 36
+    mp = _mp(G)
+    centres = [(0.25, 0.25, 0.25), (0.72, 0.3, 0.3), (0.3, 0.74, 0.66), (0.7, 0.7, 0.72)]
+    radii = [0.15, 0.12, 0.17, 0.1]
+    each = [_sphere_phi(mp, c, r) for c, r in zip(centres, radii)]
+    counts = []
+    for phi in each:
+        _, _, idx = R.mc_indexed(mp, phi)
+        label, nc, big = R.mesh_components(idx, int(idx.max()) + 1)
+        assert nc == 1 and big == idx.shape[0] and not label.any()
+        counts.append(idx.shape[0])
+    verts, _, idx = R.mc_indexed(mp, np.minimum.reduce(each))  # union of the spheres
+    label, nc, big = R.mesh_components(idx, verts.shape[0])
+    assert nc == 4 and idx.shape[0] == sum(counts) and big == max(counts)
+    per = np.bincount(label[idx[:, 0].astype(np.int64)], minlength=verts.shape[0])
+    assert sorted(per[per > 0].tolist()) == sorted(counts)
