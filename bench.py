@@ -351,7 +351,20 @@ def main():
     torch.cuda.synchronize()
     indexed = {"ms_per_pass": evi[0].elapsed_time(evi[1]) / 3, "vertices": n_iv, "triangles": n_tris,
                "what": "mc_extract_indexed: S14 + welded vertices, central-difference normals, index buffer"}
-    del iverts, inorm, iidx
+    # connectivity of that mesh (Table 2's last column under reading D:A-CONNECT): share of the largest component
+    ilabel = torch.empty(max(n_iv, 1), dtype=torch.int32, device=fr.device)
+    n_comp, largest = B.mc_mesh_components(fr.ctx, iidx, n_tris, n_iv, ilabel)
+    evc = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    evc[0].record()
+    for _ in range(3):
+        B.mc_mesh_components(fr.ctx, iidx, n_tris, n_iv, ilabel, sync=False)
+    evc[1].record()
+    torch.cuda.synchronize()
+    indexed["connectivity"] = {"components": n_comp, "largest_component_triangles": largest,
+                               "percent_connected": 100.0 * largest / max(n_tris, 1),
+                               "ms_per_pass": evc[0].elapsed_time(evc[1]) / 3,
+                               "what": "mc_mesh_components: union-find over the welded vertices"}
+    del iverts, inorm, iidx, ilabel
     # N4 baseline (not part of `value`): neighbour counts through the sorted grid (grid build + count pass) against the
     # paper's first, unsorted fixed-capacity hash grid, same positions, same counts
     cnt_a = torch.zeros(n, dtype=torch.int32, device=fr.device)

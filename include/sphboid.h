@@ -195,6 +195,17 @@ int mc_extract_indexed(sph_ctx* ctx, const mc_params* mp /* host */, void* strea
                        float* normals, uint32_t vert_capacity, uint32_t* indices, uint32_t tri_capacity,
                        uint32_t* n_verts_host, uint32_t* n_tris_host);
 
+/* N3 connectivity ("... for the triangles to connect with each other", Table 2's last column P:595-602; reading
+ * D:A-CONNECT): connected components of an indexed mesh, two triangles being connected when they share a vertex.
+ * indices = n_tris * 3 vertex ids below n_verts (DEVICE, e.g. mc_extract_indexed's output); label = n_verts words
+ * (DEVICE, out): the smallest vertex id of the vertex's component.  *n_components_host (host, optional) = number of
+ * components (a vertex no triangle uses is one, with no triangle); *largest_tris_host (host, optional) = triangles of
+ * the component that has most, so 100 * largest / n_tris is the "percent of connected triangles" under D:A-CONNECT.
+ * Passing either host pointer makes the call synchronise; an index >= n_verts is then reported as SPH_E_INVALID
+ * (the labels are unspecified in that case).  Scratch (n_verts words) is kept in the context and grows on demand. */
+int mc_mesh_components(sph_ctx* ctx, const uint32_t* indices, uint32_t n_tris, uint32_t n_verts, void* stream,
+                       uint32_t* label, uint32_t* n_components_host, uint32_t* largest_tris_host);
+
 /* End-to-end frame with HOST buffers (pinned or pageable): copies pos/vel/bpos/bvel to the device, runs
  * `steps` frames of sph_build_grid + sph_step + boid_step, optionally one surface pass on the final
  * positions (mp != NULL), copies the state (and triangles) back and synchronises.

@@ -91,6 +91,7 @@ def lib():
         L.mc_wait.argtypes = [_vp, _vp, _vp]
         L.mc_polygonise_indexed.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _u32, _vp, _u32, _vp, _vp]
         L.mc_extract_indexed.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _u32, _vp, _u32, _vp, _vp]
+        L.mc_mesh_components.argtypes = [_vp, _vp, _u32, _u32, _vp, _vp, _vp, _vp]
         L.sph_simulate_host.argtypes = [_vp, _vp, _vp, _u32, _vp, _vp, _u32, _vp, _u32, _vp, _vp, _u32, _vp]
         L.sph_mc_table.argtypes = [_vp, _vp]
         L.sph_mc_table.restype = None
@@ -105,7 +106,7 @@ def lib():
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_pack_range", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_pack_range", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "mc_mesh_components", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
            "sph_profile_read", "sph_kernel_name"]
 
 
@@ -318,6 +319,15 @@ def mc_extract_indexed(ctx, mc, verts, normals, indices, phi=None, stream=None, 
                                   C.byref(nt) if sync else None)
     _check(ctx, rc, allow=(SPH_E_CAPACITY,))
     return (int(nv.value), int(nt.value)) if sync else None
+
+
+def mc_mesh_components(ctx, indices, n_tris, n_verts, label, stream=None, sync=True):
+    """N3 connectivity: label[v] = smallest vertex id of v's component; returns (n_components, largest_tris)."""
+    nc, big = _u32(0), _u32(0)
+    rc = lib().mc_mesh_components(ctx, _ptr(indices), int(n_tris), int(n_verts), _stream(stream), _ptr(label),
+                                  C.byref(nc) if sync else None, C.byref(big) if sync else None)
+    _check(ctx, rc)
+    return (int(nc.value), int(big.value)) if sync else None
 
 
 def sph_simulate_host(ctx, pos, vel, bpos=None, bvel=None, boid=None, steps=1, mc=None, tris=None):

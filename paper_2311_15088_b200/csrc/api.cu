@@ -46,6 +46,8 @@ struct sph_ctx {
   uint32_t *pack_blocks, *pack_total;  // N2: scratch of sph_pack_range (lazy)
   uint32_t *hg_tracker, *hg_grid, *hg_dropped;  // N4 baseline: the paper's unsorted fixed-capacity hash grid (lazy)
   uint32_t hg_cap;
+  uint32_t *cc_count, *cc_result;      // N3 connectivity: per-root triangle counts (lazy, grows), result words
+  uint32_t cc_cap;
   ObstacleConst oc;      // N4: Obstacle Grid set by boid_set_obstacles (normals stay caller-owned)
   const float4* obst_normals;
   bool boid_state;       // bg/rho_bS hold the boids given to the last sph_step
@@ -339,6 +341,7 @@ int sph_destroy(sph_ctx* ctx) {
   if (ctx->ev_rho) cudaEventDestroy(ctx->ev_rho);
   cudaFree(ctx->hg_tracker), cudaFree(ctx->hg_grid), cudaFree(ctx->hg_dropped);
   cudaFree(ctx->pack_blocks), cudaFree(ctx->pack_total);
+  cudaFree(ctx->cc_count), cudaFree(ctx->cc_result);
   cudaFree(ctx->h_pos), cudaFree(ctx->h_vel), cudaFree(ctx->h_bpos), cudaFree(ctx->h_bvel), cudaFree(ctx->h_tris);
   delete ctx;
   return SPH_OK;
@@ -358,7 +361,8 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step", "k_boid_obstacles",
-    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_hashgrid_fill", "k_hashgrid_count", "k_range_count", "k_range_scan", "k_range_scatter", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32"};
+    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_hashgrid_fill", "k_hashgrid_count", "k_range_count", "k_range_scan", "k_range_scatter", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32",
+    "k_cc_init", "k_cc_link", "k_cc_flatten", "k_cc_count", "k_cc_largest"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -689,6 +693,34 @@ int mc_extract_indexed(sph_ctx* ctx, const mc_params* mp, void* stream, float* p
   if (rc != SPH_OK) return rc;
   return polygonise_indexed(ctx, mp, field, ctx->bits_ready, stream, verts, normals, vert_capacity, indices,
                             tri_capacity, n_verts_host, n_tris_host);
+}
+
+int mc_mesh_components(sph_ctx* ctx, const uint32_t* indices, uint32_t n_tris, uint32_t n_verts, void* stream,
+                       uint32_t* label, uint32_t* n_components_host, uint32_t* largest_tris_host) {
+  if (!ctx) return SPH_E_INVALID;
+  if ((n_tris > 0 && !indices) || (n_verts > 0 && !label)) return fail(ctx, SPH_E_INVALID, "indices / label is NULL");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  if (!ctx->cc_result) CK(cudaMalloc(&ctx->cc_result, 3 * 4));
+  if (n_verts > ctx->cc_cap || !ctx->cc_count) {
+    CK(cudaStreamSynchronize(s));  // an earlier call on this stream may still use the old scratch
+    cudaFree(ctx->cc_count);
+    ctx->cc_count = nullptr;
+    ctx->cc_cap = 0;
+    CK(cudaMalloc(&ctx->cc_count, (size_t)std::max<uint32_t>(n_verts, 1u) * 4));
+    ctx->cc_cap = std::max<uint32_t>(n_verts, 1u);
+  }
+  launch_mesh_components(indices, n_tris, n_verts, label, ctx->cc_count, ctx->cc_result, s, &ctx->prof);
+  CK(cudaGetLastError());
+  if (n_components_host || largest_tris_host) {
+    uint32_t r[3] = {0, 0, 0};
+    CK(cudaMemcpyAsync(r, ctx->cc_result, sizeof(r), cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    if (r[2]) return fail(ctx, SPH_E_INVALID, "vertex index out of range");
+    if (n_components_host) *n_components_host = r[0];
+    if (largest_tris_host) *largest_tris_host = r[1];
+  }
+  return SPH_OK;
 }
 
 int mc_extract(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi, float* tris, uint32_t tri_capacity,

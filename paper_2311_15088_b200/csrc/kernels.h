@@ -45,6 +45,7 @@ enum KernelId {
   K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
   K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_BOID_OBSTACLES, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
   K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_HASHGRID_FILL, K_HASHGRID_COUNT, K_RANGE_COUNT, K_RANGE_SCAN, K_RANGE_SCATTER, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_MC_EDGE_SCAN, K_MC_VERTICES, K_MC_EMIT_INDICES, K_ZERO_U32,
+  K_CC_INIT, K_CC_LINK, K_CC_FLATTEN, K_CC_COUNT, K_CC_LARGEST,  // N3 connectivity
   K_NUM_KERNELS
 };
 
@@ -132,6 +133,8 @@ void launch_mc_indexed(const McConst& m, const float* phi, uint32_t* bits, bool 
                        float* verts, float* normals, uint32_t vert_capacity, uint32_t* indices, uint32_t tri_capacity,
                        uint32_t* n_verts_dev, uint32_t* n_tris_dev, uint2* work, uint32_t* n_work, ScanState& scan,
                        cudaStream_t s, Prof* prof);
+void launch_mesh_components(const uint32_t* indices, uint32_t n_tris, uint32_t n_verts, uint32_t* label,
+                            uint32_t* tri_count, uint32_t* result /* [3] */, cudaStream_t s, Prof* prof);
 uint32_t mc_word_tiles(uint32_t G);    // look-back tiles of the edge scan
 uint64_t mc_num_segments(uint32_t G);  // size of the active-segment work list
 uint64_t mc_bits_words(uint32_t G);  // size of the corner sign bit field

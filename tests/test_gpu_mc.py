@@ -11,7 +11,7 @@ import torch
 from oracle import refbind as R
 from paper_2311_15088_b200 import binding as B
 from paper_2311_15088_b200 import workloads as W
-from tests.gpuutil import Sim, dev
+from tests.gpuutil import Sim, dev, host_u32
 
 pytestmark = pytest.mark.gpu
 
@@ -258,3 +258,71 @@ def test_indexed_extract_on_config_matches_triangle_soup():
         assert np.abs(normals.cpu().numpy()[:nv] - n_ref).max() <= 1e-5
         ln = np.linalg.norm(normals.cpu().numpy()[:nv].astype(np.float64), axis=1)
         assert np.abs(ln[ln > 0] - 1.0).max() < 1e-5
+
+
+# ---- N3 connectivity (mc_mesh_components; reading D:A-CONNECT) -------------------------------------------------------
+def _components(ctx, idx_np, n_verts):
+    idx = dev(np.ascontiguousarray(idx_np, np.uint32).view(np.int32).reshape(-1, 3)) if len(idx_np) else None
+    label = torch.full((max(n_verts, 1),), -3, dtype=torch.int32, device="cuda")
+    nc, big = B.mc_mesh_components(ctx, idx, len(idx_np), n_verts, label)
+    return host_u32(label)[:n_verts], nc, big
+
+
+def test_mesh_components_match_oracle_on_synthetic_index_buffers():
+    cfg = W.config(1)
+    rng = np.random.default_rng(5)
+    with Sim(cfg, G=8) as sim:
+        cases = []
+        for V, T in ((1, 0), (9, 0), (3, 1), (40, 9), (300, 120), (5000, 1700), (5000, 9000), (70001, 50021)):
+            cases.append((rng.integers(0, V, size=(T, 3)).astype(np.uint32), V))
+        # a long strip (the deepest trees a union-find can build), in order, reversed and shuffled
+        strip = np.stack([np.arange(0, 200000), np.arange(1, 200001), np.arange(2, 200002)], 1).astype(np.uint32)
+        cases += [(strip, 200002), (strip[::-1].copy(), 200002), (strip[rng.permutation(len(strip))], 200005)]
+        # many small components: 30 000 triangles of their own, vertex ids scattered
+        perm = rng.permutation(90000).astype(np.uint32)
+        cases.append((perm.reshape(-1, 3), 90000))
+        # scratch shrinks and grows between calls (context-owned, grows on demand)
+        for idx, V in cases + cases[:4]:
+            label, nc, big = _components(sim.ctx, idx, V)
+            l_ref, nc_ref, big_ref = R.mesh_components(idx, V)
+            assert (nc, big) == (nc_ref, big_ref)
+            assert np.array_equal(label, l_ref)
+
+
+def test_mesh_components_rejects_an_index_out_of_range():
+    cfg = W.config(1)
+    with Sim(cfg, G=8) as sim:
+        idx = np.array([[0, 1, 2], [2, 3, 9]], np.uint32)
+        with pytest.raises(Exception):
+            _components(sim.ctx, idx, 9)
+        label, nc, big = _components(sim.ctx, idx, 10)  # the context is usable afterwards
+        assert (nc, big) == (6, 2) and label.tolist() == [0, 0, 0, 0, 4, 5, 6, 7, 8, 0]
+
+
+def test_mesh_components_on_fluid_and_on_scattered_particles():
+    # a fluid config: the mesh of mc_extract_indexed; then particles further apart than 2 R: one closed blob each
+    cfg = W.config(2)
+    mp = W.mc_params(cfg)
+    G = mp["n_point_per_axis"]
+    with Sim(cfg, G=G) as sim:
+        B.sph_build_grid(sim.ctx, dev(cfg["pos"]))
+        verts = torch.zeros(400000, 3, device="cuda")
+        idx = torch.zeros(400000, 3, dtype=torch.int32, device="cuda")
+        nv, nt = B.mc_extract_indexed(sim.ctx, mp, verts, None, idx)
+        label = torch.zeros(nv, dtype=torch.int32, device="cuda")
+        nc, big = B.mc_mesh_components(sim.ctx, idx, nt, nv, label)
+        l_ref, nc_ref, big_ref = R.mesh_components(host_u32(idx)[:nt], nv)
+        assert (nc, big) == (nc_ref, big_ref) and np.array_equal(host_u32(label), l_ref)
+        assert 1 <= nc < nv and big <= nt
+        # scattered: 64 lone particles ON voxel corners 16 spacings apart: phi = -rbar at that corner, > 0 at its six
+        # neighbours, so every particle is an octahedron of 8 triangles on 6 vertices, connected to nothing else
+        g = np.array([8, 24, 40, 56], np.float32) * np.float32(mp["spacing"])
+        x, y, z = np.meshgrid(g, g, g, indexing="ij")
+        pts = np.stack([x.ravel(), y.ravel(), z.ravel(), np.zeros(64, np.float32)], 1).astype(np.float32)
+        B.sph_build_grid(sim.ctx, dev(pts))
+        nv, nt = B.mc_extract_indexed(sim.ctx, mp, verts, None, idx)
+        assert (nv, nt) == (64 * 6, 64 * 8)
+        label = torch.zeros(nv, dtype=torch.int32, device="cuda")
+        nc, big = B.mc_mesh_components(sim.ctx, idx, nt, nv, label)
+        l_ref, nc_ref, big_ref = R.mesh_components(host_u32(idx)[:nt], nv)
+        assert (nc, big) == (64, 8) == (nc_ref, big_ref) and np.array_equal(host_u32(label), l_ref)
