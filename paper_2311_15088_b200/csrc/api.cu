@@ -57,6 +57,9 @@ struct sph_ctx {
   cudaStream_t side;     // the boid grid + probe density of sph_step run here, beside k_density
   cudaStream_t surf;     // mc_extract_async runs the surface pass here, beside the next frame's SPH step
   cudaEvent_t ev_surf_fork, ev_surf_done;
+  cudaStream_t up;       // sph_simulate_host uploads the velocities here while the grid build and k_density run
+  cudaEvent_t ev_up_go, ev_up_done;
+  bool vel_pending;      // the grid was built from positions alone: sph_step gathers velS after ev_up_done
   bool surf_pending;     // a surface pass was forked and nothing has waited for it yet
   uint32_t surf_capacity;
   ScanState scan_mc;     // look-back state of the surface pass (its scans may run beside the grid scans)
@@ -233,6 +236,7 @@ int build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, cudaS
   ctx->grid_n = n;
   ctx->grid_fresh = true;
   ctx->step_state = false;
+  ctx->vel_pending = false;
   return SPH_OK;
 }
 
@@ -311,6 +315,9 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   ctx->scan.epoch = 0;
   if (cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
       cudaStreamCreateWithFlags(&ctx->surf, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&ctx->up, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_up_go, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_up_done, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_surf_fork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_surf_done, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -334,6 +341,9 @@ int sph_destroy(sph_ctx* ctx) {
   free(ctx->prof.recs);
   if (ctx->side) cudaStreamDestroy(ctx->side);
   if (ctx->surf) cudaStreamDestroy(ctx->surf);
+  if (ctx->up) cudaStreamDestroy(ctx->up);
+  if (ctx->ev_up_go) cudaEventDestroy(ctx->ev_up_go);
+  if (ctx->ev_up_done) cudaEventDestroy(ctx->ev_up_done);
   if (ctx->ev_surf_fork) cudaEventDestroy(ctx->ev_surf_fork);
   if (ctx->ev_surf_done) cudaEventDestroy(ctx->ev_surf_done);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -362,7 +372,7 @@ static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step", "k_boid_obstacles",
     "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_hashgrid_fill", "k_hashgrid_count", "k_range_count", "k_range_scan", "k_range_scatter", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32",
-    "k_cc_init", "k_cc_link", "k_cc_flatten", "k_cc_count", "k_cc_largest"};
+    "k_cc_init", "k_cc_link", "k_cc_flatten", "k_cc_count", "k_cc_largest", "k_gather_vel"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -447,6 +457,11 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     if (fork) CK(cudaEventRecord(ctx->ev_join, ctx->side));
   }
   launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, nl, s, &ctx->prof);
+  if (ctx->vel_pending) {  // sph_simulate_host: the velocities arrived on the upload stream while the above ran
+    CK(cudaStreamWaitEvent(s, ctx->ev_up_done, 0));
+    launch_gather_vel(ctx->pg, (const float4*)vel, n, s, &ctx->prof);
+    ctx->vel_pending = false;
+  }
   ctx->rho_event = n_boid > 0 && !ctx->prof.on;
   if (ctx->rho_event) {
     CK(cudaEventRecord(ctx->ev_rho, s));
@@ -789,14 +804,34 @@ int sph_simulate_host(sph_ctx* ctx, float* pos_host, float* vel_host, uint32_t n
     ctx->h_tris_cap = tri_capacity;
   }
   cudaStream_t s = nullptr;
-  CK(cudaMemcpyAsync(ctx->h_pos, pos_host, (size_t)n * 16, cudaMemcpyHostToDevice, s));
-  CK(cudaMemcpyAsync(ctx->h_vel, vel_host, (size_t)n * 16, cudaMemcpyHostToDevice, s));
+  // upload order: boids (small), positions, then the velocities on the upload stream: the first step's grid build and
+  // density pass need positions only and run while the velocities are still crossing the bus; sph_step gathers the
+  // sorted velocities (k_gather_vel) once they are there
+  const bool split = steps > 0 && n > 0;
   if (n_boid) {
     CK(cudaMemcpyAsync(ctx->h_bpos, bpos_host, (size_t)n_boid * 16, cudaMemcpyHostToDevice, s));
     CK(cudaMemcpyAsync(ctx->h_bvel, bvel_host, (size_t)n_boid * 16, cudaMemcpyHostToDevice, s));
   }
+  CK(cudaMemcpyAsync(ctx->h_pos, pos_host, (size_t)n * 16, cudaMemcpyHostToDevice, s));
+  if (split) {
+    CK(cudaEventRecord(ctx->ev_up_go, s));
+    CK(cudaStreamWaitEvent(ctx->up, ctx->ev_up_go, 0));
+    CK(cudaMemcpyAsync(ctx->h_vel, vel_host, (size_t)n * 16, cudaMemcpyHostToDevice, ctx->up));
+    CK(cudaEventRecord(ctx->ev_up_done, ctx->up));
+  } else {
+    CK(cudaMemcpyAsync(ctx->h_vel, vel_host, (size_t)n * 16, cudaMemcpyHostToDevice, s));
+  }
   for (uint32_t t = 0; t < steps; ++t) {
-    int rc = sph_build_grid(ctx, ctx->h_pos, ctx->h_vel, n, s, nullptr, nullptr, nullptr);
+    int rc;
+    if (t == 0 && split) {
+      build_grid(ctx, ctx->h_pos, nullptr, n, s);
+      CK(cudaGetLastError());
+      ctx->grid_vel = ctx->h_vel;  // sph_step below takes this grid as its own and completes velS itself
+      ctx->vel_pending = true;
+      rc = SPH_OK;
+    } else {
+      rc = sph_build_grid(ctx, ctx->h_pos, ctx->h_vel, n, s, nullptr, nullptr, nullptr);
+    }
     if (rc != SPH_OK) return rc;
     rc = sph_step(ctx, ctx->h_pos, ctx->h_vel, n, ctx->h_bpos, ctx->h_bvel, n_boid, bp, s, nullptr, nullptr, nullptr,
                   nullptr);

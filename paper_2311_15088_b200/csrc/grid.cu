@@ -175,6 +175,17 @@ __global__ void __launch_bounds__(kThreads) k_reorder(const uint32_t* __restrict
   if (vel) velS[dst] = __ldg(vel + id);
 }
 
+// The velocity half of k_reorder on its own, for a grid that was built from the positions alone while the
+// velocities were still on their way to the device (sph_simulate_host).  velS[.].w already holds rho (k_density).
+__global__ void __launch_bounds__(kThreads) k_gather_vel(const uint32_t* __restrict__ perm, const float4* __restrict__ vel,
+                                                         uint32_t n, float4* __restrict__ velS) {
+  const uint32_t s = blockIdx.x * kThreads + threadIdx.x;
+  if (s >= n) return;
+  float4 v = __ldg(vel + __ldg(perm + s));
+  v.w = velS[s].w;
+  velS[s] = v;
+}
+
 // ---- N4: the paper's FIRST neighbour search, kept as a measured baseline (K7) -------------
 // compute_hash_grid (Listing 5): hash_grid[cell * max_per_cell + slot] = particle id, slot = the cell's running count
 // (hash_grid_tracker).  Particles that find their cell full are dropped and counted (the paper leaves that case open).
@@ -301,6 +312,13 @@ void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const f
     prof->end(s);
   }
   b.aabb_now = b.aabb;
+}
+
+void launch_gather_vel(const GridBuf& b, const float4* vel, uint32_t n, cudaStream_t s, Prof* prof) {
+  if (n == 0) return;
+  prof->begin(K_GATHER_VEL, s);
+  k_gather_vel<<<(n + kThreads - 1) / kThreads, kThreads, 0, s>>>(b.perm, vel, n, b.velS);
+  prof->end(s);
 }
 
 void launch_hashgrid_count(const GridDesc& g, float h2, const float4* pos, uint32_t n, uint32_t cap, uint32_t* tracker,

@@ -125,3 +125,31 @@ def test_cuda_graph_of_pipelined_frames_matches_eager():
             want_nt, want_tris, want_pos = eager[3 * (rep + 1)]
             assert np.array_equal(fb.pos.cpu().numpy(), want_pos)
             assert np.array_equal(fb.tris[:want_nt].cpu().numpy(), want_tris)
+
+
+@pytest.mark.parametrize("pinned", [True, False])
+def test_simulate_host_three_steps_is_bitwise_the_device_path(pinned):
+    # sph_simulate_host uploads the velocities beside the first step's grid build and density pass (k_gather_vel
+    # completes the sorted copy afterwards): the state after three steps must be bit for bit what the device-resident
+    # calls give, with pinned and with pageable host buffers
+    from paper_2311_15088_b200.pipeline import Frame
+    cfg = W.config(2, scale=2)
+    with Frame(cfg) as fr:
+        for _ in range(3):
+            fr.sim()
+        want = [t.cpu().numpy().copy() for t in (fr.pos, fr.vel, fr.bpos, fr.bvel)]
+
+    def host(a):
+        t = torch.from_numpy(np.ascontiguousarray(a).copy())
+        return t.pin_memory() if pinned else t
+
+    got = [host(cfg[k]) for k in ("pos", "vel", "bpos", "bvel")]
+    with Sim(cfg, G=0) as sim:
+        B.sph_simulate_host(sim.ctx, got[0], got[1], got[2], got[3], cfg["boid"], 3, None, None)
+        for g, w, what in zip(got, want, ("pos", "vel", "bpos", "bvel")):
+            assert np.array_equal(g.numpy(), w), what
+        # zero steps: the state makes the round trip unchanged
+        again = [host(cfg[k]) for k in ("pos", "vel", "bpos", "bvel")]
+        B.sph_simulate_host(sim.ctx, again[0], again[1], again[2], again[3], cfg["boid"], 0, None, None)
+        for g, k in zip(again, ("pos", "vel", "bpos", "bvel")):
+            assert np.array_equal(g.numpy(), np.ascontiguousarray(cfg[k]))
