@@ -171,8 +171,8 @@ def run_reference(args, cfg_idx):
 
 
 def run_slab(args):
-    """--decomposition slab (N2): the fluid of the workload cut into slabs over the ranks, strong scaling; SPH step only
-    (boids and the surface pass are not decomposed).  Exchange: neighbour send / receive over NCCL."""
+    """--decomposition slab (N2): the fluid and the boids of the workload cut into slabs over the ranks, strong scaling;
+    SPH step + boid step (the surface pass is not decomposed).  Exchange: neighbour send / receive over NCCL."""
     import torch
     from paper_2311_15088_b200 import binding as B
     from paper_2311_15088_b200 import dist as D
@@ -186,12 +186,14 @@ def run_slab(args):
     torch.cuda.set_device(dev)
     cfg = W.config(args.config)
     n, K = cfg["n"], args.steps
-    lay = S.SlabLayout(cfg["sph"], ranks.world)
+    lay = S.SlabLayout(cfg["sph"], ranks.world, boid=cfg["boid"])
     p, v = S.split_initial(lay, cfg["pos"], cfg["vel"])[ranks.rank]
-    be = S.GpuBackend(cfg["sph"], min(n, 2 * (n // ranks.world) + (1 << 16)), device=dev)
+    bp, bv = S.split_initial(lay, cfg["bpos"], cfg["bvel"])[ranks.rank]
+    be = S.GpuBackend(cfg["sph"], min(n, 2 * (n // ranks.world) + (1 << 16)), device=dev, boid_capacity=cfg["n_boid"])
     ex = (S.DistExchange(ranks.dist, ranks.rank, ranks.world, torch.device("cuda", dev)) if ranks.world > 1
           else S.LoopbackExchange(1))
-    sim = S.SlabSim(lay, ranks.rank, be, ex, be.to_device(p), be.to_device(v))
+    sim = S.SlabSim(lay, ranks.rank, be, ex, be.to_device(p), be.to_device(v), be.to_device(bp), be.to_device(bv),
+                    cfg["boid"])
     for _ in range(max(args.warmup, 3)):
         sim.step()
     sampler = ClockSampler(dev)
@@ -214,13 +216,14 @@ def run_slab(args):
     owned = ranks.reduce_max([float(sim.n_owned), float(sim.stats["ghosts"])])
     if ranks.rank == 0:
         print(json.dumps({
-            "metric": "particle-updates/s (SPH step of the fluid, slab-decomposed over the ranks; no boids, no surface pass)",
+            "metric": "particle-updates/s (SPH step + boid step, fluid and boids slab-decomposed over the ranks; no surface pass)",
             "value": n * K / t_max, "unit": "particle-updates/s", "n_gpus": ranks.world, "steps": K,
             "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_max / K, "higher_is_better": True, "scaling": "strong",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": cfg["name"], "particles": n, "parallelism": "slab x%d along axis %d" % (ranks.world, lay.axis),
                        "max_owned_per_rank": int(owned[0]), "max_ghosts_per_rank": int(owned[1]),
-                       "exchange": "2 neighbour send/recv pairs per step (halo of 2 h, migration), NCCL"},
+                       "boids": cfg["n_boid"],
+                       "exchange": "4 neighbour send/recv pairs per step (fluid halo, boid halo, two migrations), NCCL"},
             "gpu_launches": launches, "clocks": clocks, "e2e": None, "roofline": None, "cpu_baseline": None}))
     be.close()
     ranks.close()

@@ -15,9 +15,16 @@ scheme here is the standard one for a short-range particle method:
 
 Exchange steps: two neighbour send / receive pairs per step (halo, migration), variable-size; no global collective.
 This module is orchestration only: selection and packing run in libsphboid (sph_pack_range), the step is sph_step,
-torch.distributed (NCCL on GPUs, gloo in the CPU tests) moves the packed buffers.  Boids and the surface pass are not
-decomposed here (boids would be replicated with an all-reduce of the fluid->boid force; the voxel grid would be cut
-along the same axis): the decomposed run is fluid only.
+torch.distributed (NCCL on GPUs, gloo in the CPU tests) moves the packed buffers.
+
+Boids are decomposed the same way (optional: pass bpos / bvel / boid): a rank owns the boids inside its slab, receives
+ghost boids within max(visible, protect, push radius) of its faces, runs the unmodified sph_step + boid_step on
+[owned | ghost] fluid and [owned | ghost] boids, keeps the owned results and lets boids that crossed a face migrate.
+With boids the fluid halo is max(2 h, push radius + h): a ghost boid up to the push radius beyond the face pushes owned
+fluid and needs its own probe density (fluid within h of it), and a ghost particle up to the push radius beyond the
+face pushes an owned boid and needs its own density.  Every owned particle and boid then sees exactly the neighbours
+of the undecomposed run; no collective is needed.  The surface pass is not decomposed (the voxel grid would be cut
+along the same axis).
 
 The exchange is pluggable (`Exchange`): `DistExchange` uses torch.distributed; `LoopbackExchange` connects several
 domains inside ONE process (the single-GPU emulation the GPU test uses: ranks run one after the other, never
@@ -31,15 +38,20 @@ import numpy as np
 class SlabLayout:
     """Which rank owns which x-range (pure host logic, no device)."""
 
-    def __init__(self, sph, world, axis=None):
+    def __init__(self, sph, world, axis=None, boid=None):
         lo, hi = np.asarray(sph["box_min"], np.float64), np.asarray(sph["box_max"], np.float64)
         self.h = float(sph["h"])
         self.axis = int(np.argmax(hi - lo)) if axis is None else int(axis)
         self.world = int(world)
         self.dim = max(1, int(math.ceil((hi[self.axis] - lo[self.axis]) / self.h)))
         self.cells_per_rank = int(math.ceil(self.dim / self.world))
-        if self.world > 1 and self.cells_per_rank < 2:
-            raise ValueError("slabs must be at least 2 h wide (ghost layers of neighbours must not overlap)")
+        self.fluid_halo = 2.0 * self.h
+        self.boid_halo = 0.0
+        if boid is not None:
+            self.fluid_halo = max(2.0 * self.h, float(boid["push_radius"]) + self.h)
+            self.boid_halo = max(float(boid["visible_range"]), float(boid["protect_range"]), float(boid["push_radius"]))
+        if self.world > 1 and self.cells_per_rank * self.h < max(self.fluid_halo, self.boid_halo):
+            raise ValueError("slabs must be at least one halo wide (ghosts come from the two neighbours only)")
         self.origin = float(np.float32(lo[self.axis]))
         # faces in binary32, the precision positions are compared in
         self.faces = [float(np.float32(self.origin + np.float32(self.cells_per_rank * r) * np.float32(self.h)))
@@ -57,7 +69,10 @@ class SlabLayout:
         return np.searchsorted(np.asarray(self.faces, np.float32), x, side="right").astype(np.int64)
 
     def halo_width(self):
-        return float(np.float32(2.0) * np.float32(self.h))
+        return float(np.float32(self.fluid_halo))
+
+    def boid_halo_width(self):
+        return float(np.float32(self.boid_halo))
 
 
 class LoopbackExchange:
@@ -132,14 +147,14 @@ class DistExchange:
 class GpuBackend:
     """Selection and stepping through libsphboid on one GPU (device memory from torch)."""
 
-    def __init__(self, sph, capacity, device=0):
+    def __init__(self, sph, capacity, device=0, boid_capacity=1):
         import torch
         from . import binding as B
         self.B, self.torch = B, torch
         self.device = torch.device("cuda", device)
         torch.cuda.set_device(self.device)
         self.capacity = int(capacity)
-        self.ctx = B.sph_create(sph, self.capacity, 1, 0, device=device)
+        self.ctx = B.sph_create(sph, self.capacity, max(int(boid_capacity), 1), 0, device=device)
         self.scratch = [torch.empty(self.capacity, 4, device=self.device) for _ in range(2)]
 
     def to_device(self, a):
@@ -147,14 +162,23 @@ class GpuBackend:
 
     def pack(self, pos, vel, n, axis, lo, hi):
         """Ordered copy of the particles of the first n with lo <= x < hi -> (pos, vel) tensors (fresh storage)."""
+        if n == 0:
+            return self.empty(), self.empty()
         k = self.B.sph_pack_range(self.ctx, pos, vel, n, axis, lo, hi, self.scratch[0], self.scratch[1])
         return self.scratch[0][:k].clone(), self.scratch[1][:k].clone()
 
-    def step(self, pos, vel):
-        self.B.sph_step(self.ctx, pos, vel)
+    def step(self, pos, vel, bpos=None, bvel=None, boid=None):
+        if bpos is None or bpos.shape[0] == 0:
+            self.B.sph_step(self.ctx, pos, vel)
+        else:
+            self.B.sph_step(self.ctx, pos, vel, bpos, bvel, boid)
+            self.B.boid_step(self.ctx, boid, bpos, bvel)
 
     def cat(self, parts):
         return self.torch.cat(parts, 0) if len(parts) > 1 else parts[0]
+
+    def empty(self):
+        return self.torch.empty(0, 4, device=self.device)
 
     def close(self):
         if self.ctx is not None:
@@ -163,50 +187,88 @@ class GpuBackend:
 
 
 class SlabSim:
-    """One rank of the decomposed fluid.  pos / vel: this rank's OWNED particles ((n, 4) tensors of the backend)."""
+    """One rank of the decomposed run.  pos / vel: this rank's OWNED particles ((n, 4) tensors of the backend);
+    bpos / bvel / boid (optional): its OWNED boids and the boid parameters."""
 
-    def __init__(self, layout, rank, backend, exchange, pos, vel):
+    def __init__(self, layout, rank, backend, exchange, pos, vel, bpos=None, bvel=None, boid=None):
         self.layout, self.rank, self.backend, self.exchange = layout, rank, backend, exchange
         self.lo, self.hi = layout.bounds(rank)
         self.pos, self.vel = pos, vel
         self.n_owned = pos.shape[0]
-        self.halo = layout.halo_width() * 1.001  # a little over 2 h: the pair predicate is evaluated in binary32
+        self.boid = boid
+        self.bpos, self.bvel = bpos, bvel
+        self.nb_owned = 0 if bpos is None else bpos.shape[0]
+        if boid is not None and layout.boid_halo <= 0.0:
+            raise ValueError("the layout was made without the boid parameters")
+        # a little over the nominal widths: the pair predicates are evaluated in binary32
+        self.halo = layout.halo_width() * 1.001
+        self.bhalo = layout.boid_halo_width() * 1.001
         self.step_no = 0
-        self.stats = dict(ghosts=0, migrated_out=0)
+        self.stats = dict(ghosts=0, migrated_out=0, boid_ghosts=0, boids_migrated_out=0)
+
+    def _faces(self, pos, vel, n, width):
+        """(to_left, to_right): the first n rows within `width` of the lower / upper face."""
+        ax, be = self.layout.axis, self.backend
+        to_left = be.pack(pos, vel, n, ax, self.lo, self.lo + width) if self.rank > 0 else None
+        to_right = be.pack(pos, vel, n, ax, self.hi - width, self.hi) if self.rank < self.layout.world - 1 else None
+        return to_left, to_right
+
+    def _leavers(self, pos, vel, n):
+        """(go_left, go_right, stay) of the first n rows."""
+        ax, be, inf = self.layout.axis, self.backend, math.inf
+        go_left = be.pack(pos, vel, n, ax, -inf, self.lo) if self.rank > 0 else None
+        go_right = be.pack(pos, vel, n, ax, self.hi, inf) if self.rank < self.layout.world - 1 else None
+        return go_left, go_right, be.pack(pos, vel, n, ax, self.lo, self.hi)
+
+    @staticmethod
+    def _nonempty(parts):
+        return [g for g in parts if g is not None and g[0].shape[0] > 0]
 
     # -- phase 1: halo ---------------------------------------------------------------------------------------------
     def post_halo(self):
-        ax, be = self.layout.axis, self.backend
-        to_left = be.pack(self.pos, self.vel, self.n_owned, ax, self.lo, self.lo + self.halo) if self.rank > 0 else None
-        to_right = (be.pack(self.pos, self.vel, self.n_owned, ax, self.hi - self.halo, self.hi)
-                    if self.rank < self.layout.world - 1 else None)
-        self.exchange.post(self.rank, ("halo", self.step_no), to_left, to_right)
+        self.exchange.post(self.rank, ("halo", self.step_no), *self._faces(self.pos, self.vel, self.n_owned, self.halo))
+        if self.boid is not None:
+            self.exchange.post(self.rank, ("bhalo", self.step_no),
+                               *self._faces(self.bpos, self.bvel, self.nb_owned, self.bhalo))
 
     def step_with_halo(self):
-        from_left, from_right = self.exchange.collect(self.rank, ("halo", self.step_no))
-        ghosts = [g for g in (from_left, from_right) if g is not None and g[0].shape[0] > 0]
-        pos_all = self.backend.cat([self.pos] + [g[0] for g in ghosts])
-        vel_all = self.backend.cat([self.vel] + [g[1] for g in ghosts])
+        be = self.backend
+        ghosts = self._nonempty(self.exchange.collect(self.rank, ("halo", self.step_no)))
+        pos_all = be.cat([self.pos] + [g[0] for g in ghosts])
+        vel_all = be.cat([self.vel] + [g[1] for g in ghosts])
         self.stats["ghosts"] = pos_all.shape[0] - self.n_owned
-        self.backend.step(pos_all, vel_all)  # in place; the ghosts' results are not used
+        if self.boid is None:
+            be.step(pos_all, vel_all)  # in place; the ghosts' results are not used
+        else:
+            bghosts = self._nonempty(self.exchange.collect(self.rank, ("bhalo", self.step_no)))
+            bpos_all = be.cat([self.bpos] + [g[0] for g in bghosts])
+            bvel_all = be.cat([self.bvel] + [g[1] for g in bghosts])
+            self.stats["boid_ghosts"] = bpos_all.shape[0] - self.nb_owned
+            be.step(pos_all, vel_all, bpos_all, bvel_all, self.boid)
+            self.bpos, self.bvel = bpos_all[:self.nb_owned], bvel_all[:self.nb_owned]
         self.pos, self.vel = pos_all[:self.n_owned], vel_all[:self.n_owned]
 
     # -- phase 2: migration ----------------------------------------------------------------------------------------
     def post_migration(self):
-        ax, be = self.layout.axis, self.backend
-        inf = math.inf
-        go_left = be.pack(self.pos, self.vel, self.n_owned, ax, -inf, self.lo) if self.rank > 0 else None
-        go_right = be.pack(self.pos, self.vel, self.n_owned, ax, self.hi, inf) if self.rank < self.layout.world - 1 else None
-        self._stay = be.pack(self.pos, self.vel, self.n_owned, ax, self.lo, self.hi)
+        go_left, go_right, self._stay = self._leavers(self.pos, self.vel, self.n_owned)
         self.stats["migrated_out"] = self.n_owned - self._stay[0].shape[0]
         self.exchange.post(self.rank, ("move", self.step_no), go_left, go_right)
+        if self.boid is not None:
+            go_left, go_right, self._bstay = self._leavers(self.bpos, self.bvel, self.nb_owned)
+            self.stats["boids_migrated_out"] = self.nb_owned - self._bstay[0].shape[0]
+            self.exchange.post(self.rank, ("bmove", self.step_no), go_left, go_right)
 
     def finish_migration(self):
-        from_left, from_right = self.exchange.collect(self.rank, ("move", self.step_no))
-        parts = [self._stay] + [g for g in (from_left, from_right) if g is not None and g[0].shape[0] > 0]
-        self.pos = self.backend.cat([p[0] for p in parts])
-        self.vel = self.backend.cat([p[1] for p in parts])
+        be = self.backend
+        parts = [self._stay] + self._nonempty(self.exchange.collect(self.rank, ("move", self.step_no)))
+        self.pos = be.cat([p[0] for p in parts])
+        self.vel = be.cat([p[1] for p in parts])
         self.n_owned = self.pos.shape[0]
+        if self.boid is not None:
+            parts = [self._bstay] + self._nonempty(self.exchange.collect(self.rank, ("bmove", self.step_no)))
+            self.bpos = be.cat([p[0] for p in parts])
+            self.bvel = be.cat([p[1] for p in parts])
+            self.nb_owned = self.bpos.shape[0]
         self.step_no += 1
 
     def step(self):

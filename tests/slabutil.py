@@ -15,13 +15,25 @@ class OracleBackend:
     def to_device(self, a):
         return torch.from_numpy(np.ascontiguousarray(a, np.float32).copy())
 
+    def empty(self):
+        return torch.empty(0, 4)
+
     def pack(self, pos, vel, n, axis, lo, hi):
+        if n == 0:
+            return self.empty(), self.empty()
         x = pos[:n, axis].numpy()
         sel = torch.from_numpy((x >= np.float32(lo)) & (x < np.float32(hi)))
         return pos[:n][sel].clone(), vel[:n][sel].clone()
 
-    def step(self, pos, vel):
-        out = R.step(self.sph, pos.numpy(), vel.numpy())
+    def step(self, pos, vel, bpos=None, bvel=None, boid=None):
+        if bpos is None or bpos.shape[0] == 0:
+            out = R.step(self.sph, pos.numpy(), vel.numpy())
+        else:
+            p0, v0 = pos.numpy().copy(), vel.numpy().copy()
+            out = R.step(self.sph, p0, v0, bpos.numpy(), bvel.numpy(), boid)
+            ob = R.boid_step(self.sph, boid, p0, v0, out["density"], bpos.numpy(), bvel.numpy())
+            bpos.copy_(torch.from_numpy(ob["bpos"]))
+            bvel.copy_(torch.from_numpy(ob["bvel"]))
         pos.copy_(torch.from_numpy(out["pos"]))
         vel.copy_(torch.from_numpy(out["vel"]))
 
@@ -50,3 +62,23 @@ def gather_by_id(parts, n):
     assert ids.shape[0] == n and np.array_equal(np.sort(ids), np.arange(n)), "particles lost or duplicated"
     order = np.argsort(ids)
     return pos[order], vel[order]
+
+
+def tagged_boids(cfg, seed=9, speed=25.0):
+    """Boids of the config with the boid id in bpos.w (carried through by boid_step), velocities and a speed cap that
+    carry boids across slab faces within a few steps.  Returns (bpos, bvel, boid params)."""
+    from paper_2311_15088_b200 import workloads as W
+    nb = cfg["n_boid"]
+    bpos = cfg["bpos"].copy()
+    bpos[:, 3] = np.arange(nb, dtype=np.float32)
+    bvel = W.uniform_box(nb, (-speed,) * 3, (speed,) * 3, seed, 31)
+    return bpos, bvel, dict(cfg["boid"], max_speed=2.0 * speed)
+
+
+def reference_frames(cfg, pos, vel, bpos, bvel, boid, steps):
+    """The undecomposed oracle: `steps` frames of step + boid_step.  Returns (pos, vel, bpos, bvel)."""
+    for _ in range(steps):
+        o = R.step(cfg["sph"], pos, vel, bpos, bvel, boid)
+        ob = R.boid_step(cfg["sph"], boid, pos, vel, o["density"], bpos, bvel)
+        pos, vel, bpos, bvel = o["pos"], o["vel"], ob["bpos"], ob["bvel"]
+    return pos, vel, bpos, bvel

@@ -78,3 +78,41 @@ def test_slab_decomposed_steps_match_undecomposed_oracle(idx, scale, world):
     finally:
         for b in backends:
             b.close()
+
+
+@pytest.mark.parametrize("idx,scale,world", [(1, None, 3), (2, None, 3), (2, None, 4)])
+def test_slab_decomposed_frames_with_boids_match_undecomposed_oracle(idx, scale, world):
+    # fluid and boids both cut into slabs (ghost boids; fluid halo push radius + h): sph_step + boid_step per emulated
+    # rank, against the undecomposed oracle frames, particle by particle and boid by boid
+    from tests.slabutil import reference_frames, tagged_boids
+    cfg = W.config(idx, scale=scale)
+    pos, vel = tagged_state(cfg, speed=8.0)
+    bpos, bvel, boid = tagged_boids(cfg)
+    n, nb, steps = cfg["n"], cfg["n_boid"], 3
+    lay = S.SlabLayout(cfg["sph"], world, boid=boid)
+    ex = S.LoopbackExchange(world)
+    backends = [S.GpuBackend(cfg["sph"], n, boid_capacity=nb) for _ in range(world)]
+    try:
+        fluid, boids = S.split_initial(lay, pos, vel), S.split_initial(lay, bpos, bvel)
+        sims = [S.SlabSim(lay, r, backends[r], ex, backends[r].to_device(fluid[r][0]), backends[r].to_device(fluid[r][1]),
+                          backends[r].to_device(boids[r][0]), backends[r].to_device(boids[r][1]), boid)
+                for r in range(world)]
+        moved = ghosts = 0
+        for s in range(steps):
+            S.run_loopback(sims, 1)
+            moved += sum(x.stats["boids_migrated_out"] for x in sims)
+            ghosts += sum(x.stats["boid_ghosts"] for x in sims)
+            for x in sims:
+                xs = x.bpos[:, lay.axis]
+                assert bool(((xs >= x.lo) & (xs < x.hi)).all())
+        assert moved > 0 and ghosts > 0
+        rp, rv, rbp, rbv = reference_frames(cfg, pos, vel, bpos, bvel, boid, steps)
+        gp, gv = gather_by_id([(x.pos.cpu().numpy(), x.vel.cpu().numpy()) for x in sims], n)
+        gbp, gbv = gather_by_id([(x.bpos.cpu().numpy(), x.bvel.cpu().numpy()) for x in sims], nb)
+        for got, want, what, abs_ in ((gp, rp, "pos", 2e-6), (gv, rv, "vel", 2e-5), (gbp, rbp, "bpos", 2e-6),
+                                      (gbv, rbv, "bvel", 1e-4)):
+            bad, worst = vec_err(got[:, :3], want[:, :3], rel=1e-5 * steps, abs_=abs_ * steps)
+            assert bad <= got.shape[0] // 10000, (what, bad, worst)
+    finally:
+        for b in backends:
+            b.close()

@@ -55,6 +55,47 @@ def test_loopback_decomposition_equals_undecomposed_oracle():
     assert np.abs(gp[:, :3] - rp[:, :3]).max() <= 1e-6 and np.abs(gv[:, :3] - rv[:, :3]).max() <= 1e-5
 
 
+
+def test_loopback_decomposition_with_boids_equals_undecomposed_oracle():
+    # fluid AND boids cut into slabs (ghost boids, wider fluid halo: push radius + h), oracle as the stepper: every
+    # particle and every boid ends where the undecomposed oracle frames put it; boids migrate too
+    from tests.slabutil import OracleBackend, gather_by_id, reference_frames, tagged_boids, tagged_state
+    cfg = W.config(1)
+    pos, vel = tagged_state(cfg)
+    bpos, bvel, boid = tagged_boids(cfg)
+    world = 3
+    lay = S.SlabLayout(cfg["sph"], world, boid=boid)
+    assert lay.halo_width() >= boid["push_radius"] + cfg["sph"]["h"] - 1e-6 and lay.boid_halo_width() >= boid["visible_range"]
+    ex = S.LoopbackExchange(world)
+    be = OracleBackend(cfg["sph"])
+    fluid = S.split_initial(lay, pos, vel)
+    boids = S.split_initial(lay, bpos, bvel)
+    sims = [S.SlabSim(lay, r, be, ex, be.to_device(fluid[r][0]), be.to_device(fluid[r][1]), be.to_device(boids[r][0]),
+                      be.to_device(boids[r][1]), boid) for r in range(world)]
+    steps, moved = 4, 0
+    for _ in range(steps):
+        S.run_loopback(sims, 1)
+        moved += sum(s.stats["boids_migrated_out"] for s in sims)
+        for s in sims:
+            x = s.bpos[:, lay.axis].numpy()
+            assert ((x >= np.float32(s.lo)) & (x < np.float32(s.hi))).all()
+    assert moved > 0 and sum(s.stats["boid_ghosts"] for s in sims) > 0
+    rp, rv, rbp, rbv = reference_frames(cfg, pos, vel, bpos, bvel, boid, steps)
+    gp, gv = gather_by_id([(s.pos.numpy(), s.vel.numpy()) for s in sims], cfg["n"])
+    gbp, gbv = gather_by_id([(s.bpos.numpy(), s.bvel.numpy()) for s in sims], cfg["n_boid"])
+    assert np.abs(gp[:, :3] - rp[:, :3]).max() <= 1e-6 and np.abs(gv[:, :3] - rv[:, :3]).max() <= 1e-5
+    assert np.abs(gbp[:, :3] - rbp[:, :3]).max() <= 1e-6 and np.abs(gbv[:, :3] - rbv[:, :3]).max() <= 2e-5
+
+
+def test_slab_layout_rejects_slabs_narrower_than_a_halo():
+    import pytest
+    cfg = W.config(1)  # 16 cells of h along x; visible range 0.1 = 1.6 h, push radius h: fluid halo 2 h, boid halo 1.6 h
+    S.SlabLayout(cfg["sph"], 8, boid=cfg["boid"])  # 2 cells per rank: just wide enough
+    with pytest.raises(ValueError):
+        S.SlabLayout(cfg["sph"], 16, boid=cfg["boid"])
+    with pytest.raises(ValueError):
+        S.SlabLayout(cfg["sph"], 8, boid=dict(cfg["boid"], push_radius=2.0 * cfg["sph"]["h"]))  # fluid halo 3 h
+
 _WORKER = r"""
 import os, sys
 sys.path.insert(0, {root!r})
@@ -66,36 +107,70 @@ rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
 dist.init_process_group("gloo", rank=rank, world_size=world)
 cfg = W.config(1)
 pos, vel = tagged_state(cfg)
-lay = S.SlabLayout(cfg["sph"], world)
 be = OracleBackend(cfg["sph"])
-p, v = S.split_initial(lay, pos, vel)[rank]
-sim = S.SlabSim(lay, rank, be, S.DistExchange(dist, rank, world, torch.device("cpu")), be.to_device(p), be.to_device(v))
+ex = S.DistExchange(dist, rank, world, torch.device("cpu"))
+if os.environ.get("SLAB_BOIDS") == "1":
+    from tests.slabutil import tagged_boids
+    bpos, bvel, boid = tagged_boids(cfg)
+    lay = S.SlabLayout(cfg["sph"], world, boid=boid)
+    p, v = S.split_initial(lay, pos, vel)[rank]
+    bp, bv = S.split_initial(lay, bpos, bvel)[rank]
+    sim = S.SlabSim(lay, rank, be, ex, be.to_device(p), be.to_device(v), be.to_device(bp), be.to_device(bv), boid)
+else:
+    lay = S.SlabLayout(cfg["sph"], world)
+    p, v = S.split_initial(lay, pos, vel)[rank]
+    sim = S.SlabSim(lay, rank, be, ex, be.to_device(p), be.to_device(v))
 for _ in range(3):
     sim.step()
 np.save({out!r} % rank, np.concatenate([sim.pos.numpy(), sim.vel.numpy()], 1))
+if sim.boid is not None:
+    np.save({bout!r} % rank, np.concatenate([sim.bpos.numpy(), sim.bvel.numpy()], 1))
 dist.barrier()
 dist.destroy_process_group()
 print("rank", rank, "ok", sim.n_owned, sim.stats)
 """
 
 
-def test_decomposed_step_under_gloo_world_size_2(tmp_path):
-    from oracle import refbind as R
-    from tests.slabutil import gather_by_id, tagged_state
+def _run_world2(tmp_path, boids):
     script = tmp_path / "worker.py"
-    out_pat = str(tmp_path / "rank%d.npy")
-    script.write_text(_WORKER.format(root=ROOT, out=out_pat))
-    port = 29900 + os.getpid() % 90
+    out_pat, bout_pat = str(tmp_path / "rank%d.npy"), str(tmp_path / "boids%d.npy")
+    script.write_text(_WORKER.format(root=ROOT, out=out_pat, bout=bout_pat))
+    port = 29900 + (os.getpid() + (45 if boids else 0)) % 90
     procs = []
     for rank in range(2):
         env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
-                   MASTER_PORT=str(port), CUDA_VISIBLE_DEVICES="", OMP_NUM_THREADS="2")
+                   MASTER_PORT=str(port), CUDA_VISIBLE_DEVICES="", OMP_NUM_THREADS="2", SLAB_BOIDS="1" if boids else "0")
         procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
                                       stderr=subprocess.STDOUT, text=True))
     for rank, p in enumerate(procs):
         out, _ = p.communicate(timeout=300)
         assert p.returncode == 0, out
         assert "rank %d ok" % rank in out
+    return out_pat, bout_pat
+
+
+def test_decomposed_frames_with_boids_under_gloo_world_size_2(tmp_path):
+    from tests.slabutil import gather_by_id, reference_frames, tagged_boids, tagged_state
+    out_pat, bout_pat = _run_world2(tmp_path, True)
+    cfg = W.config(1)
+    pos, vel = tagged_state(cfg)
+    bpos, bvel, boid = tagged_boids(cfg)
+    rp, rv, rbp, rbv = reference_frames(cfg, pos, vel, bpos, bvel, boid, 3)
+    parts, bparts = [], []
+    for rank in range(2):
+        a, b = np.load(out_pat % rank), np.load(bout_pat % rank)
+        parts.append((a[:, :4], a[:, 4:]))
+        bparts.append((b[:, :4], b[:, 4:]))
+    gp, gv = gather_by_id(parts, cfg["n"])
+    gbp, gbv = gather_by_id(bparts, cfg["n_boid"])
+    assert np.abs(gp[:, :3] - rp[:, :3]).max() <= 1e-6 and np.abs(gv[:, :3] - rv[:, :3]).max() <= 1e-5
+    assert np.abs(gbp[:, :3] - rbp[:, :3]).max() <= 1e-6 and np.abs(gbv[:, :3] - rbv[:, :3]).max() <= 2e-5
+
+
+def test_decomposed_step_under_gloo_world_size_2(tmp_path):
+    from oracle import refbind as R
+    from tests.slabutil import gather_by_id, tagged_state
+    out_pat, _ = _run_world2(tmp_path, False)
     cfg = W.config(1)
     rp, rv = tagged_state(cfg)
     for _ in range(3):
