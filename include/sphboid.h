@@ -150,6 +150,14 @@ int sph_set_force_variant(sph_ctx* ctx, int variant);
  * positions to mesh) else SPH_E_STALE_GRID.  phi[G^3]. */
 int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, float* phi);
 
+/* Restrict S15-S17 (mc_polygonise, mc_extract, their async / indexed forms) to the cubes whose index along `axis`
+ * is in [lo, hi) (clamped to the grid); the other two axes keep their ranges; axis = -1 resets all three to the whole
+ * grid (the default).  Triangles keep the order of D:A-APPEND among the cubes that remain, so the meshes of a partition
+ * of the cubes add up to the mesh of the whole grid.  Used by the slab decomposition: a rank
+ * polygonises the cubes of its own slab from its own and its ghost particles.  phi, the sign field and the vertices of
+ * the indexed form still cover the whole grid.  Host-side setting, takes effect with the next call. */
+int mc_set_cube_range(sph_ctx* ctx, int axis, uint32_t lo, uint32_t hi);
+
 /* S14 has four kernels that compute the same phi: 1 = one thread per corner, 2 = a warp per
  * group of particle cells, 3 = a warp per block of 4x4x2 corners with a filtered candidate list, 4 = a warp per tile
  * of 8x8x4 corners, 2x2x2 corners per lane, with per-lane candidate lists.  0 (default) picks by a cost model from the

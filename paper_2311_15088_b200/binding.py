@@ -80,6 +80,7 @@ def lib():
         L.boid_step.argtypes = [_vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.mc_voxel_sdf.argtypes = [_vp, _vp, _vp, _vp]
         L.mc_set_sdf_variant.argtypes = [_vp, C.c_int]
+        L.mc_set_cube_range.argtypes = [_vp, C.c_int, _u32, _u32]
         L.boid_set_obstacles.argtypes = [_vp, _vp, _vp]
         L.sph_neighbor_count.argtypes = [_vp, _vp, _u32, _vp, _vp]
         L.sph_pack_range.argtypes = [_vp, _vp, _vp, _u32, C.c_int, _f, _f, _vp, _vp, _vp, _u32, _vp]
@@ -106,7 +107,7 @@ def lib():
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "mc_voxel_sdf", "mc_set_sdf_variant", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_pack_range", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "mc_mesh_components", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "mc_voxel_sdf", "mc_set_sdf_variant", "mc_set_cube_range", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_pack_range", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "mc_mesh_components", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
            "sph_profile_read", "sph_kernel_name"]
 
 
@@ -255,6 +256,11 @@ def sph_hashgrid_neighbor_count(ctx, pos, max_per_cell, ncount, stream=None, syn
 
 def sph_set_force_variant(ctx, variant):
     return _check(ctx, lib().sph_set_force_variant(ctx, int(variant)))
+
+
+def mc_set_cube_range(ctx, axis, lo=0, hi=0xffffffff):
+    """Polygonise only the cubes with lo <= index < hi along axis (axis = -1: the whole grid again)."""
+    return _check(ctx, lib().mc_set_cube_range(ctx, int(axis), int(lo), int(hi)))
 
 
 def mc_set_sdf_variant(ctx, variant):

@@ -27,6 +27,7 @@ struct sph_ctx {
   uint32_t sdf_first_cap;
   NbrList nbr;           // stored neighbour list of the last sph_step
   int force_variant;     // 0 = stored neighbour list (k_force_list), 1 = grid walk (k_force_integrate)
+  uint32_t cube_lo[3], cube_hi[3];  // mc_set_cube_range: cubes the polygoniser handles (default: all)
   int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = cell groups, 3 = corner blocks, 4 = corner tiles (mc_set_sdf_variant)
   uint32_t* n_tris_dev;
   uint32_t* mc_prefix;   // [words of mc_bits] vertex-id prefix of the indexed mesh (N3)
@@ -224,6 +225,7 @@ int make_mc(sph_ctx* ctx, const mc_params* mp, McConst& m) {
   m.iso = mp->iso;
   int r = (int)ceil((double)mp->radius / (double)ctx->p.h);  // D:A-R
   m.reach = r < 1 ? 1 : r;
+  for (int a = 0; a < 3; ++a) m.cube_lo[a] = ctx->cube_lo[a], m.cube_hi[a] = ctx->cube_hi[a];
   return SPH_OK;
 }
 
@@ -253,6 +255,7 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
   sph_ctx* ctx = new (std::nothrow) sph_ctx();
   if (!ctx) return SPH_E_CUDA;
   memset(ctx, 0, sizeof(*ctx));
+  for (int a = 0; a < 3; ++a) ctx->cube_hi[a] = 0xffffffffu;
   ctx->device = device;
   ctx->p = *p;
   SphConst& sc = ctx->sc;
@@ -554,6 +557,16 @@ int boid_set_obstacles(sph_ctx* ctx, const obstacle_params* op, const void* norm
   ctx->oc.w_obs = op->w_obs;
   ctx->oc.heavy = op->heavy;
   ctx->obst_normals = (const float4*)normals;
+  return SPH_OK;
+}
+
+int mc_set_cube_range(sph_ctx* ctx, int axis, uint32_t lo, uint32_t hi) {
+  if (!ctx) return SPH_E_INVALID;
+  if (axis < -1 || axis > 2) return fail(ctx, SPH_E_INVALID, "axis must be -1 (reset), 0, 1 or 2");
+  if (axis >= 0 && lo > hi) return fail(ctx, SPH_E_INVALID, "empty ranges are lo == hi, not lo > hi");
+  for (int a = 0; a < 3; ++a)
+    if (axis < 0) ctx->cube_lo[a] = 0u, ctx->cube_hi[a] = 0xffffffffu;
+    else if (a == axis) ctx->cube_lo[a] = lo, ctx->cube_hi[a] = hi;
   return SPH_OK;
 }
 

@@ -37,6 +37,7 @@ struct McConst {
   uint32_t G;
   float R, R2, rbar, iso;
   int reach;            // ceil(R / h) particle cells (D:A-R)
+  uint32_t cube_lo[3], cube_hi[3];  // cubes that are polygonised: lo <= index < hi per axis (mc_set_cube_range)
 };
 
 // Kernel ids for the per-kernel timing that bench.py's roofline object is built from (sph_profile_*).

@@ -326,3 +326,47 @@ def test_mesh_components_on_fluid_and_on_scattered_particles():
         nc, big = B.mc_mesh_components(sim.ctx, idx, nt, nv, label)
         l_ref, nc_ref, big_ref = R.mesh_components(host_u32(idx)[:nt], nv)
         assert (nc, big) == (64, 8) == (nc_ref, big_ref) and np.array_equal(host_u32(label), l_ref)
+
+
+# ---- cube ranges (mc_set_cube_range; the surface pass of the slab decomposition) ---------------------
+def test_polygonise_cube_ranges_are_the_ordered_subsets_of_the_whole_mesh():
+    # white noise on 70^3 corners (69 cubes per axis: segments of 32, 32 and 5 cubes).  The oracle gives every
+    # triangle's cube (cube-major order, ntri[case] triangles each); a cube range must return exactly the triangles of
+    # the cubes inside it, in the same order, bit for bit; a partition of an axis adds up to the whole mesh
+    G = 70
+    Q = G - 1
+    rng = np.random.default_rng(17)
+    phi = rng.standard_normal(G ** 3).astype(np.float32)
+    mp = dict(origin=(0.1, -0.2, 0.3), spacing=0.013, n_point_per_axis=G, radius=0.05, particle_radius=0.02, iso=0.3)
+    tris_ref, nt_ref, cases = R.mc_polygonise(mp, phi, want_cases=True)
+    _, ntri, _ = R.mc_table()
+    cube_of_tri = np.repeat(np.arange(Q ** 3), ntri[cases].astype(np.int64))
+    assert cube_of_tri.shape[0] == nt_ref
+    ci, cj, ck = cube_of_tri % Q, (cube_of_tri // Q) % Q, cube_of_tri // (Q * Q)
+    coord = (ci, cj, ck)
+    cfg = dict(sph=W.config(1)["sph"], n=1)
+    with Sim(cfg, G=G) as sim:
+        def run(ranges):
+            B.mc_set_cube_range(sim.ctx, -1)
+            keep = np.ones(nt_ref, bool)
+            for axis, lo, hi in ranges:
+                B.mc_set_cube_range(sim.ctx, axis, lo, hi)
+                keep &= (coord[axis] >= lo) & (coord[axis] < hi)
+            tris, nt = _polygonise_gpu(sim, mp, phi, nt_ref)
+            assert nt == int(keep.sum()), ranges
+            assert np.array_equal(tris[:nt], tris_ref[keep]), ranges
+            return nt
+
+        for ranges in ([(0, 0, 7)], [(0, 7, 40)], [(0, 31, 33)], [(0, 64, 1000)], [(0, 5, 5)], [(1, 3, 21)], [(2, 60, 69)],
+                       [(0, 10, 50), (1, 0, 30), (2, 17, 18)], [(0, 33, 64), (2, 0, 0)]):
+            run(ranges)
+        for axis in range(3):  # a partition into four slabs adds up to the whole
+            cuts = [0, 13, 32, 51, Q]
+            assert sum(run([(axis, cuts[r], cuts[r + 1])]) for r in range(4)) == nt_ref
+        B.mc_set_cube_range(sim.ctx, -1)
+        tris, nt = _polygonise_gpu(sim, mp, phi, nt_ref)
+        assert nt == nt_ref and np.array_equal(tris, tris_ref)
+        with pytest.raises(B.SphError):
+            B.mc_set_cube_range(sim.ctx, 0, 5, 4)
+        with pytest.raises(B.SphError):
+            B.mc_set_cube_range(sim.ctx, 3, 0, 4)
