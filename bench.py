@@ -171,8 +171,9 @@ def run_reference(args, cfg_idx):
 
 
 def run_slab(args):
-    """--decomposition slab (N2): the fluid and the boids of the workload cut into slabs over the ranks, strong scaling;
-    SPH step + boid step (the surface pass is not decomposed).  Exchange: neighbour send / receive over NCCL."""
+    """--decomposition slab (N2): the fluid, the boids and the cubes of the voxel grid cut into slabs over the ranks,
+    strong scaling; a step is the whole frame (surface pass of the frame-start state for the rank's cubes, SPH step,
+    boid step).  Exchange: neighbour send / receive over NCCL; one all-reduce of the triangle counts at the end."""
     import torch
     from paper_2311_15088_b200 import binding as B
     from paper_2311_15088_b200 import dist as D
@@ -186,16 +187,19 @@ def run_slab(args):
     torch.cuda.set_device(dev)
     cfg = W.config(args.config)
     n, K = cfg["n"], args.steps
-    lay = S.SlabLayout(cfg["sph"], ranks.world, boid=cfg["boid"])
+    mc = W.mc_params(cfg)
+    lay = S.SlabLayout(cfg["sph"], ranks.world, boid=cfg["boid"], mc=mc)
     p, v = S.split_initial(lay, cfg["pos"], cfg["vel"])[ranks.rank]
     bp, bv = S.split_initial(lay, cfg["bpos"], cfg["bvel"])[ranks.rank]
-    be = S.GpuBackend(cfg["sph"], min(n, 2 * (n // ranks.world) + (1 << 16)), device=dev, boid_capacity=cfg["n_boid"])
+    be = S.GpuBackend(cfg["sph"], min(n, 2 * (n // ranks.world) + (1 << 16)), device=dev, boid_capacity=cfg["n_boid"],
+                      mc_points=mc["n_point_per_axis"])
     ex = (S.DistExchange(ranks.dist, ranks.rank, ranks.world, torch.device("cuda", dev)) if ranks.world > 1
           else S.LoopbackExchange(1))
     sim = S.SlabSim(lay, ranks.rank, be, ex, be.to_device(p), be.to_device(v), be.to_device(bp), be.to_device(bv),
                     cfg["boid"])
+    tris = torch.empty(max(1 << 16, (4 << 20) // ranks.world), 3, 3, device=torch.device("cuda", dev))
     for _ in range(max(args.warmup, 3)):
-        sim.step()
+        sim.step(tris)
     sampler = ClockSampler(dev)
     sampler.start()
     time.sleep(0.15)
@@ -204,25 +208,30 @@ def run_slab(args):
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
     launches0 = B.sph_launch_count(be.ctx)
     ev[0].record()
+    n_tris = 0
     for _ in range(K):
-        sim.step()
+        n_tris = sim.step(tris)
     ev[1].record()
     torch.cuda.synchronize()
     ranks.barrier()
+    if n_tris > tris.shape[0]:
+        raise SystemExit("triangle buffer too small: %d > %d" % (n_tris, tris.shape[0]))
     t = ev[0].elapsed_time(ev[1]) * 1e-3
     launches = B.sph_launch_count(be.ctx) - launches0
     clocks = sampler.stop()
     t_max, _ = ranks.combine(t, 0.0)
     owned = ranks.reduce_max([float(sim.n_owned), float(sim.stats["ghosts"])])
+    _, tris_total = ranks.combine(0.0, float(n_tris))
     if ranks.rank == 0:
         print(json.dumps({
-            "metric": "particle-updates/s (SPH step + boid step, fluid and boids slab-decomposed over the ranks; no surface pass)",
+            "metric": "particle-updates/s (whole frame, slab-decomposed over the ranks: surface pass of the rank's cubes, SPH step, boid step)",
             "value": n * K / t_max, "unit": "particle-updates/s", "n_gpus": ranks.world, "steps": K,
             "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_max / K, "higher_is_better": True, "scaling": "strong",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": cfg["name"], "particles": n, "parallelism": "slab x%d along axis %d" % (ranks.world, lay.axis),
                        "max_owned_per_rank": int(owned[0]), "max_ghosts_per_rank": int(owned[1]),
-                       "boids": cfg["n_boid"],
+                       "boids": cfg["n_boid"], "mc_points_per_axis": mc["n_point_per_axis"],
+                       "triangles_last_frame": int(tris_total),
                        "exchange": "4 neighbour send/recv pairs per step (fluid halo, boid halo, two migrations), NCCL"},
             "gpu_launches": launches, "clocks": clocks, "e2e": None, "roofline": None, "cpu_baseline": None}))
     be.close()

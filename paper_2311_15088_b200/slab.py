@@ -23,8 +23,14 @@ ghost boids within max(visible, protect, push radius) of its faces, runs the unm
 With boids the fluid halo is max(2 h, push radius + h): a ghost boid up to the push radius beyond the face pushes owned
 fluid and needs its own probe density (fluid within h of it), and a ghost particle up to the push radius beyond the
 face pushes an owned boid and needs its own density.  Every owned particle and boid then sees exactly the neighbours
-of the undecomposed run; no collective is needed.  The surface pass is not decomposed (the voxel grid would be cut
-along the same axis).
+of the undecomposed run; no collective is needed.
+
+The surface pass is decomposed by cubes (optional: pass mc to the layout): the voxel grid is the global one on every
+rank; a rank polygonises the cubes whose lower corner lies in its slab (mc_set_cube_range) from [owned | ghost]
+particles, which requires a fluid halo of R + one voxel spacing (the upper corners of its last cubes lie up to one
+spacing beyond the face, and phi there needs the particles within R).  The ranks' triangle lists add up to the mesh of
+the undecomposed run (each is that mesh's ordered subset for the rank's cubes); an all-gather of the counts would give
+output offsets where one buffer is wanted.
 
 The exchange is pluggable (`Exchange`): `DistExchange` uses torch.distributed; `LoopbackExchange` connects several
 domains inside ONE process (the single-GPU emulation the GPU test uses: ranks run one after the other, never
@@ -38,7 +44,7 @@ import numpy as np
 class SlabLayout:
     """Which rank owns which x-range (pure host logic, no device)."""
 
-    def __init__(self, sph, world, axis=None, boid=None):
+    def __init__(self, sph, world, axis=None, boid=None, mc=None):
         lo, hi = np.asarray(sph["box_min"], np.float64), np.asarray(sph["box_max"], np.float64)
         self.h = float(sph["h"])
         self.axis = int(np.argmax(hi - lo)) if axis is None else int(axis)
@@ -50,6 +56,9 @@ class SlabLayout:
         if boid is not None:
             self.fluid_halo = max(2.0 * self.h, float(boid["push_radius"]) + self.h)
             self.boid_halo = max(float(boid["visible_range"]), float(boid["protect_range"]), float(boid["push_radius"]))
+        self.mc = mc
+        if mc is not None:
+            self.fluid_halo = max(self.fluid_halo, float(mc["radius"]) + float(mc["spacing"]))
         if self.world > 1 and self.cells_per_rank * self.h < max(self.fluid_halo, self.boid_halo):
             raise ValueError("slabs must be at least one halo wide (ghosts come from the two neighbours only)")
         self.origin = float(np.float32(lo[self.axis]))
@@ -67,6 +76,16 @@ class SlabLayout:
         """Rank that owns coordinate(s) x (numpy, binary32 comparison)."""
         x = np.asarray(x, np.float32)
         return np.searchsorted(np.asarray(self.faces, np.float32), x, side="right").astype(np.int64)
+
+    def cube_range(self, rank):
+        """[i0, i1): the cubes (by index along the slab axis) whose lower corner lies in rank's slab; corner
+        coordinates in binary32 as the kernels form them (origin + i * spacing)."""
+        mc = self.mc
+        q = int(mc["n_point_per_axis"]) - 1
+        x = np.float32(mc["origin"][self.axis]) + np.arange(q, dtype=np.float32) * np.float32(mc["spacing"])
+        lo, hi = self.bounds(rank)
+        return (int(np.searchsorted(x, np.float32(lo), side="left")) if rank > 0 else 0,
+                int(np.searchsorted(x, np.float32(hi), side="left")) if rank < self.world - 1 else q)
 
     def halo_width(self):
         return float(np.float32(self.fluid_halo))
@@ -147,14 +166,14 @@ class DistExchange:
 class GpuBackend:
     """Selection and stepping through libsphboid on one GPU (device memory from torch)."""
 
-    def __init__(self, sph, capacity, device=0, boid_capacity=1):
+    def __init__(self, sph, capacity, device=0, boid_capacity=1, mc_points=0):
         import torch
         from . import binding as B
         self.B, self.torch = B, torch
         self.device = torch.device("cuda", device)
         torch.cuda.set_device(self.device)
         self.capacity = int(capacity)
-        self.ctx = B.sph_create(sph, self.capacity, max(int(boid_capacity), 1), 0, device=device)
+        self.ctx = B.sph_create(sph, self.capacity, max(int(boid_capacity), 1), int(mc_points), device=device)
         self.scratch = [torch.empty(self.capacity, 4, device=self.device) for _ in range(2)]
 
     def to_device(self, a):
@@ -173,6 +192,15 @@ class GpuBackend:
         else:
             self.B.sph_step(self.ctx, pos, vel, bpos, bvel, boid)
             self.B.boid_step(self.ctx, boid, bpos, bvel)
+
+    def surface(self, pos, vel, mc, axis, lo, hi, tris):
+        """S14-S17 on these particles for the cubes lo <= index < hi along axis; returns the triangle count.  The grid
+        it builds is the one the following step on the same (pos, vel) reuses."""
+        B = self.B
+        B.mc_set_cube_range(self.ctx, -1)
+        B.mc_set_cube_range(self.ctx, axis, lo, hi)
+        B.sph_build_grid(self.ctx, pos, vel)
+        return B.mc_extract(self.ctx, mc, tris)
 
     def cat(self, parts):
         return self.torch.cat(parts, 0) if len(parts) > 1 else parts[0]
@@ -231,22 +259,37 @@ class SlabSim:
             self.exchange.post(self.rank, ("bhalo", self.step_no),
                                *self._faces(self.bpos, self.bvel, self.nb_owned, self.bhalo))
 
-    def step_with_halo(self):
+    def collect_halo(self):
+        """[owned | ghosts] of this frame (fluid, and boids when present)."""
         be = self.backend
         ghosts = self._nonempty(self.exchange.collect(self.rank, ("halo", self.step_no)))
-        pos_all = be.cat([self.pos] + [g[0] for g in ghosts])
-        vel_all = be.cat([self.vel] + [g[1] for g in ghosts])
-        self.stats["ghosts"] = pos_all.shape[0] - self.n_owned
-        if self.boid is None:
-            be.step(pos_all, vel_all)  # in place; the ghosts' results are not used
-        else:
+        self._all = [be.cat([self.pos] + [g[0] for g in ghosts]), be.cat([self.vel] + [g[1] for g in ghosts])]
+        self.stats["ghosts"] = self._all[0].shape[0] - self.n_owned
+        if self.boid is not None:
             bghosts = self._nonempty(self.exchange.collect(self.rank, ("bhalo", self.step_no)))
-            bpos_all = be.cat([self.bpos] + [g[0] for g in bghosts])
-            bvel_all = be.cat([self.bvel] + [g[1] for g in bghosts])
-            self.stats["boid_ghosts"] = bpos_all.shape[0] - self.nb_owned
-            be.step(pos_all, vel_all, bpos_all, bvel_all, self.boid)
-            self.bpos, self.bvel = bpos_all[:self.nb_owned], bvel_all[:self.nb_owned]
-        self.pos, self.vel = pos_all[:self.n_owned], vel_all[:self.n_owned]
+            self._all += [be.cat([self.bpos] + [g[0] for g in bghosts]), be.cat([self.bvel] + [g[1] for g in bghosts])]
+            self.stats["boid_ghosts"] = self._all[2].shape[0] - self.nb_owned
+
+    def surface(self, tris):
+        """The surface of the CURRENT state for this rank's cubes (between collect_halo and step_collected).  Returns
+        the triangle count; tris holds them in the order of the undecomposed mesh."""
+        lay = self.layout
+        i0, i1 = lay.cube_range(self.rank)
+        return self.backend.surface(self._all[0], self._all[1], lay.mc, lay.axis, i0, i1, tris)
+
+    def step_collected(self):
+        be = self.backend
+        if self.boid is None:
+            be.step(self._all[0], self._all[1])  # in place; the ghosts' results are not used
+        else:
+            be.step(self._all[0], self._all[1], self._all[2], self._all[3], self.boid)
+            self.bpos, self.bvel = self._all[2][:self.nb_owned], self._all[3][:self.nb_owned]
+        self.pos, self.vel = self._all[0][:self.n_owned], self._all[1][:self.n_owned]
+        self._all = None
+
+    def step_with_halo(self):
+        self.collect_halo()
+        self.step_collected()
 
     # -- phase 2: migration ----------------------------------------------------------------------------------------
     def post_migration(self):
@@ -271,12 +314,16 @@ class SlabSim:
             self.nb_owned = self.bpos.shape[0]
         self.step_no += 1
 
-    def step(self):
-        """One decomposed step (with DistExchange every rank calls this; with LoopbackExchange drive the phases)."""
+    def step(self, tris=None):
+        """One decomposed frame (with DistExchange every rank calls this; with LoopbackExchange drive the phases).
+        With tris: the surface of the frame-start state for this rank's cubes first; returns its triangle count."""
         self.post_halo()
-        self.step_with_halo()
+        self.collect_halo()
+        nt = self.surface(tris) if tris is not None else None
+        self.step_collected()
         self.post_migration()
         self.finish_migration()
+        return nt
 
 
 def split_initial(layout, pos, vel):
@@ -285,14 +332,21 @@ def split_initial(layout, pos, vel):
     return [(np.ascontiguousarray(pos[own == r]), np.ascontiguousarray(vel[own == r])) for r in range(layout.world)]
 
 
-def run_loopback(sims, steps):
-    """Single-process emulation: all ranks post, then all ranks collect, phase by phase."""
+def run_loopback(sims, steps, tris=None):
+    """Single-process emulation: all ranks post, then all ranks collect, phase by phase.  tris: one triangle buffer
+    per rank -> the surface pass of every frame-start state runs too; returns the counts of the last frame."""
+    counts = None
     for _ in range(steps):
         for s in sims:
             s.post_halo()
         for s in sims:
-            s.step_with_halo()
+            s.collect_halo()
+        if tris is not None:
+            counts = [s.surface(t) for s, t in zip(sims, tris)]
+        for s in sims:
+            s.step_collected()
         for s in sims:
             s.post_migration()
         for s in sims:
             s.finish_migration()
+    return counts

@@ -37,6 +37,14 @@ class OracleBackend:
         pos.copy_(torch.from_numpy(out["pos"]))
         vel.copy_(torch.from_numpy(out["vel"]))
 
+    def surface(self, pos, vel, mc, axis, lo, hi, tris):
+        phi = R.voxel_sdf(self.sph, mc, pos.numpy())
+        t, nt, cases = R.mc_polygonise(mc, phi, want_cases=True)
+        keep = triangles_in_cube_range(mc, cases, axis, lo, hi)
+        k = int(keep.sum())
+        tris[:k] = torch.from_numpy(t[keep])
+        return k
+
     def cat(self, parts):
         return torch.cat(parts, 0) if len(parts) > 1 else parts[0].clone()
 
@@ -82,3 +90,12 @@ def reference_frames(cfg, pos, vel, bpos, bvel, boid, steps):
         ob = R.boid_step(cfg["sph"], boid, pos, vel, o["density"], bpos, bvel)
         pos, vel, bpos, bvel = o["pos"], o["vel"], ob["bpos"], ob["bvel"]
     return pos, vel, bpos, bvel
+
+
+def triangles_in_cube_range(mc, cases, axis, lo, hi):
+    """Mask over the oracle's triangle list (cube-major, ntri[case] triangles per cube): cubes with lo <= index < hi."""
+    q = int(mc["n_point_per_axis"]) - 1
+    _, ntri, _ = R.mc_table()
+    cube = np.repeat(np.arange(q ** 3), ntri[cases].astype(np.int64))
+    c = (cube % q, (cube // q) % q, cube // (q * q))[axis]
+    return (c >= lo) & (c < hi)

@@ -116,3 +116,50 @@ def test_slab_decomposed_frames_with_boids_match_undecomposed_oracle(idx, scale,
     finally:
         for b in backends:
             b.close()
+
+
+@pytest.mark.parametrize("idx,scale,world", [(1, None, 3), (2, None, 2), (3, 2, 4)])
+def test_slab_decomposed_surface_matches_the_undecomposed_pass(idx, scale, world):
+    # every emulated rank polygonises the cubes of its slab (mc_set_cube_range) from [owned | ghost] particles; against
+    # (a) the same cube range polygonised by ONE context that holds all particles (same kernels; phi differs only by
+    # the order of the binary32 sums) and (b) the oracle's mesh of the gathered state, restricted to the rank's cubes
+    from tests.slabutil import triangles_in_cube_range
+    cfg = W.config(idx, scale=scale)
+    mc = W.mc_params(cfg)
+    G, h = mc["n_point_per_axis"], cfg["sph"]["h"]
+    pos, vel = tagged_state(cfg, speed=8.0)
+    n = cfg["n"]
+    lay = S.SlabLayout(cfg["sph"], world, mc=mc)
+    ex = S.LoopbackExchange(world)
+    backends = [S.GpuBackend(cfg["sph"], n, mc_points=G) for _ in range(world)]
+    try:
+        sims = [S.SlabSim(lay, r, backends[r], ex, backends[r].to_device(p), backends[r].to_device(v))
+                for r, (p, v) in enumerate(S.split_initial(lay, pos, vel))]
+        bufs = [torch.zeros(300000, 3, 3, device="cuda") for _ in range(world)]
+        S.run_loopback(sims, 2)
+        state, svel = gather_by_id([(x.pos.cpu().numpy(), x.vel.cpu().numpy()) for x in sims], n)
+        counts = S.run_loopback(sims, 1, tris=bufs)
+        phi_ref = R.voxel_sdf(cfg["sph"], mc, state)
+        t_ref, nt_ref, cases = R.mc_polygonise(mc, phi_ref, want_cases=True)
+        risky = int((np.abs(phi_ref - mc["iso"]) <= 1e-5 * h).sum())
+        assert abs(sum(counts) - nt_ref) <= 5 * 8 * risky and sum(counts) > 0
+        with Sim(cfg, G=G) as one:
+            B.sph_build_grid(one.ctx, dev(state))
+            whole = torch.zeros(300000, 3, 3, device="cuda")
+            for r in range(world):
+                i0, i1 = lay.cube_range(r)
+                B.mc_set_cube_range(one.ctx, lay.axis, i0, i1)
+                nt = B.mc_extract(one.ctx, mc, whole)
+                assert abs(nt - counts[r]) <= 5 * 8 * risky
+                keep = triangles_in_cube_range(mc, cases, lay.axis, i0, i1)
+                assert abs(int(keep.sum()) - counts[r]) <= 5 * 8 * risky
+                if nt == counts[r] and nt > 0:
+                    d = (whole[:nt] - bufs[r][:nt]).abs().flatten().cpu().numpy()
+                    assert np.quantile(d, 0.999) <= 1e-3 * mc["spacing"], (r, float(d.max()))
+                if int(keep.sum()) == counts[r] and counts[r] > 0:
+                    d = np.abs(bufs[r][:counts[r]].cpu().numpy() - t_ref[keep]).ravel()
+                    assert np.quantile(d, 0.999) <= 1e-3 * mc["spacing"], (r, float(d.max()))
+        assert sum(c > 0 for c in counts) >= 2
+    finally:
+        for b in backends:
+            b.close()

@@ -96,6 +96,38 @@ def test_slab_layout_rejects_slabs_narrower_than_a_halo():
     with pytest.raises(ValueError):
         S.SlabLayout(cfg["sph"], 8, boid=dict(cfg["boid"], push_radius=2.0 * cfg["sph"]["h"]))  # fluid halo 3 h
 
+
+def test_loopback_decomposed_surface_adds_up_to_the_undecomposed_mesh():
+    # three emulated ranks, oracle as the stepper and as the mesher: every rank polygonises the cubes of its slab from
+    # [owned | ghost] particles; each list is the undecomposed mesh's ordered subset for those cubes
+    import torch
+    from oracle import refbind as R
+    from tests.slabutil import OracleBackend, gather_by_id, tagged_state, triangles_in_cube_range
+    cfg = W.config(1)
+    mc = W.mc_params(cfg)
+    pos, vel = tagged_state(cfg)
+    world = 3
+    lay = S.SlabLayout(cfg["sph"], world, mc=mc)
+    assert lay.halo_width() >= mc["radius"] + mc["spacing"] - 1e-7
+    q = mc["n_point_per_axis"] - 1
+    rng = [lay.cube_range(r) for r in range(world)]
+    assert rng[0][0] == 0 and rng[-1][1] == q and all(rng[r][1] == rng[r + 1][0] for r in range(world - 1))
+    ex = S.LoopbackExchange(world)
+    be = OracleBackend(cfg["sph"])
+    sims = [S.SlabSim(lay, r, be, ex, be.to_device(p), be.to_device(v)) for r, (p, v) in enumerate(S.split_initial(lay, pos, vel))]
+    bufs = [torch.zeros(20000, 3, 3) for _ in range(world)]
+    S.run_loopback(sims, 2)  # two frames without the surface pass (particles migrate), then one with it
+    state = gather_by_id([(s.pos.numpy(), s.vel.numpy()) for s in sims], cfg["n"])[0]
+    counts = S.run_loopback(sims, 1, tris=bufs)
+    phi = R.voxel_sdf(cfg["sph"], mc, state)
+    t_ref, nt_ref, cases = R.mc_polygonise(mc, phi, want_cases=True)
+    assert sum(counts) == nt_ref and nt_ref > 0 and min(counts[:2]) > 0
+    for r in range(world):
+        keep = triangles_in_cube_range(mc, cases, lay.axis, *rng[r])
+        assert counts[r] == int(keep.sum())
+        if counts[r]:
+            assert np.abs(bufs[r].numpy()[:counts[r]] - t_ref[keep]).max() <= 1e-6
+
 _WORKER = r"""
 import os, sys
 sys.path.insert(0, {root!r})
