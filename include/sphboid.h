@@ -154,8 +154,10 @@ int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, flo
  * is in [lo, hi) (clamped to the grid); the other two axes keep their ranges; axis = -1 resets all three to the whole
  * grid (the default).  Triangles keep the order of D:A-APPEND among the cubes that remain, so the meshes of a partition
  * of the cubes add up to the mesh of the whole grid.  Used by the slab decomposition: a rank
- * polygonises the cubes of its own slab from its own and its ghost particles.  phi, the sign field and the vertices of
- * the indexed form still cover the whole grid.  Host-side setting, takes effect with the next call. */
+ * polygonises the cubes of its own slab from its own and its ghost particles.  The vertices of the indexed form still
+ * cover the whole grid.  S14 may skip what the range does not need: on fine grids (the corner-tile kernel) phi and the
+ * sign field are only written for the 8 x 8 x 4 corner tiles that hold corners of the cubes in range, the rest of a phi
+ * buffer keeps its old contents.  Host-side setting, takes effect with the next call. */
 int mc_set_cube_range(sph_ctx* ctx, int axis, uint32_t lo, uint32_t hi);
 
 /* S14 has four kernels that compute the same phi: 1 = one thread per corner, 2 = a warp per

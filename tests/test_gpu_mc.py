@@ -370,3 +370,48 @@ def test_polygonise_cube_ranges_are_the_ordered_subsets_of_the_whole_mesh():
             B.mc_set_cube_range(sim.ctx, 0, 5, 4)
         with pytest.raises(B.SphError):
             B.mc_set_cube_range(sim.ctx, 3, 0, 4)
+
+
+def test_extract_with_cube_ranges_on_the_tile_kernel_skips_tiles_but_not_triangles():
+    # S14 -> S17 with the corner-tile kernel forced: under a cube range only the tiles holding corners of those cubes
+    # are computed (the rest of phi keeps the NaN it was filled with), and the triangles are bit for bit the subset of
+    # the unrestricted pass for those cubes
+    from tests.slabutil import triangles_in_cube_range
+    cfg = W.config(2)
+    mp = W.mc_params(cfg)
+    G = mp["n_point_per_axis"]
+    Q = G - 1
+    with Sim(cfg, G=G) as sim:
+        B.mc_set_sdf_variant(sim.ctx, 4)
+        B.sph_build_grid(sim.ctx, dev(cfg["pos"]))
+        full = torch.zeros(400000, 3, 3, device="cuda")
+        phi = torch.zeros(G ** 3, device="cuda")
+        nt_full = B.mc_extract(sim.ctx, mp, full, phi=phi)
+        phi_np = phi.cpu().numpy()
+        t_ref, nt_ref, cases = R.mc_polygonise(mp, phi_np, want_cases=True)
+        assert nt_ref == nt_full and np.array_equal(full.cpu().numpy()[:nt_full], t_ref)
+        for ranges in ([(0, 10, 30)], [(1, 0, 9)], [(2, 50, 63)], [(0, 8, 16), (2, 4, 8)], [(0, 62, 63)], [(1, 7, 7)]):
+            B.mc_set_cube_range(sim.ctx, -1)
+            keep = np.ones(nt_full, bool)
+            needed = np.ones((G, G, G), bool)  # [k, j, i]: corners of the cubes in range
+            for axis, lo, hi in ranges:
+                B.mc_set_cube_range(sim.ctx, axis, lo, hi)
+                keep &= triangles_in_cube_range(mp, cases, axis, lo, hi)
+                idx = np.arange(G)
+                sel = (idx >= lo) & (idx <= hi) if hi > lo else np.zeros(G, bool)
+                shape = [1, 1, 1]
+                shape[2 - axis] = G
+                needed &= sel.reshape(shape)
+            part = torch.zeros(400000, 3, 3, device="cuda")
+            phi2 = torch.full((G ** 3,), float("nan"), device="cuda")
+            nt = B.mc_extract(sim.ctx, mp, part, phi=phi2)
+            assert nt == int(keep.sum()), ranges
+            assert np.array_equal(part.cpu().numpy()[:nt], t_ref[keep]), ranges
+            p2 = phi2.cpu().numpy().reshape(G, G, G)
+            written = ~np.isnan(p2)
+            assert np.array_equal(p2[written], phi_np.reshape(G, G, G)[written])
+            assert bool(written[needed].all()), ranges            # every corner a cube in range uses was computed
+            assert written.sum() < G ** 3, ranges                 # and tiles outside the range were skipped
+        B.mc_set_cube_range(sim.ctx, -1)
+        again = torch.zeros(400000, 3, 3, device="cuda")
+        assert B.mc_extract(sim.ctx, mp, again) == nt_full and bool((again[:nt_full] == full[:nt_full]).all())
