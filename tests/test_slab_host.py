@@ -144,7 +144,7 @@ ex = S.DistExchange(dist, rank, world, torch.device("cpu"))
 if os.environ.get("SLAB_BOIDS") == "1":
     from tests.slabutil import tagged_boids
     bpos, bvel, boid = tagged_boids(cfg)
-    lay = S.SlabLayout(cfg["sph"], world, boid=boid)
+    lay = S.SlabLayout(cfg["sph"], world, boid=boid, mc=W.mc_params(cfg))
     p, v = S.split_initial(lay, pos, vel)[rank]
     bp, bv = S.split_initial(lay, bpos, bvel)[rank]
     sim = S.SlabSim(lay, rank, be, ex, be.to_device(p), be.to_device(v), be.to_device(bp), be.to_device(bv), boid)
@@ -157,6 +157,10 @@ for _ in range(3):
 np.save({out!r} % rank, np.concatenate([sim.pos.numpy(), sim.vel.numpy()], 1))
 if sim.boid is not None:
     np.save({bout!r} % rank, np.concatenate([sim.bpos.numpy(), sim.bvel.numpy()], 1))
+    # a fourth frame with the surface pass of its start state (the state saved above) for this rank's cubes
+    tris = torch.zeros(20000, 3, 3)
+    nt = sim.step(tris)
+    np.save({tout!r} % rank, tris.numpy()[:nt])
 dist.barrier()
 dist.destroy_process_group()
 print("rank", rank, "ok", sim.n_owned, sim.stats)
@@ -166,7 +170,7 @@ print("rank", rank, "ok", sim.n_owned, sim.stats)
 def _run_world2(tmp_path, boids):
     script = tmp_path / "worker.py"
     out_pat, bout_pat = str(tmp_path / "rank%d.npy"), str(tmp_path / "boids%d.npy")
-    script.write_text(_WORKER.format(root=ROOT, out=out_pat, bout=bout_pat))
+    script.write_text(_WORKER.format(root=ROOT, out=out_pat, bout=bout_pat, tout=str(tmp_path / "tris%d.npy")))
     port = 29900 + (os.getpid() + (45 if boids else 0)) % 90
     procs = []
     for rank in range(2):
@@ -197,6 +201,20 @@ def test_decomposed_frames_with_boids_under_gloo_world_size_2(tmp_path):
     gbp, gbv = gather_by_id(bparts, cfg["n_boid"])
     assert np.abs(gp[:, :3] - rp[:, :3]).max() <= 1e-6 and np.abs(gv[:, :3] - rv[:, :3]).max() <= 1e-5
     assert np.abs(gbp[:, :3] - rbp[:, :3]).max() <= 1e-6 and np.abs(gbv[:, :3] - rbv[:, :3]).max() <= 2e-5
+    # the surface pass of the two ranks: each the ordered subset of the mesh of the gathered state for its cubes
+    from oracle import refbind as R
+    from tests.slabutil import triangles_in_cube_range
+    mc = W.mc_params(cfg)
+    lay = S.SlabLayout(cfg["sph"], 2, boid=boid, mc=mc)
+    t_ref, nt_ref, cases = R.mc_polygonise(mc, R.voxel_sdf(cfg["sph"], mc, gp), want_cases=True)
+    total = 0
+    for rank in range(2):
+        t = np.load(str(tmp_path / "tris%d.npy") % rank)
+        keep = triangles_in_cube_range(mc, cases, lay.axis, *lay.cube_range(rank))
+        assert t.shape[0] == int(keep.sum()) and t.shape[0] > 0
+        assert np.abs(t - t_ref[keep]).max() <= 1e-6
+        total += t.shape[0]
+    assert total == nt_ref
 
 
 def test_decomposed_step_under_gloo_world_size_2(tmp_path):
