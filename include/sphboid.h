@@ -142,7 +142,9 @@ int sph_hashgrid_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, uint3
 
 /* S8 has two kernels that compute the same forces: 0 (default) = the density pass stores each
  * particle's neighbour list (the paper's section 9 design) and the force pass reads it; 1 = the force pass
- * walks the 27 cells again.  Tests and A/B measurements force one. */
+ * walks the 27 cells again; 2 = as 0, with the list and the densities produced by k_density_pairs (two particles of a
+ * cell per thread; same results bit for bit, measured A/B in DESIGN.md section 10).  Tests and A/B measurements force
+ * one.  Any other value: SPH_E_INVALID. */
 int sph_set_force_variant(sph_ctx* ctx, int variant);
 
 /* S14: voxel signed distance phi(x) = |x - xbar| - rbar, xbar the kernel-weighted mean neighbour position

@@ -26,7 +26,7 @@ struct sph_ctx {
   uint32_t* sdf_first;  // corner partition tables of the surface pass (SdfPlan::first)
   uint32_t sdf_first_cap;
   NbrList nbr;           // stored neighbour list of the last sph_step
-  int force_variant;     // 0 = stored neighbour list (k_force_list), 1 = grid walk (k_force_integrate)
+  int force_variant;     // 0 = stored neighbour list (k_force_list), 1 = grid walk (k_force_integrate), 2 = list built by k_density_pairs
   uint32_t cube_lo[3], cube_hi[3];  // mc_set_cube_range: cubes the polygoniser handles (default: all)
   int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = cell groups, 3 = corner blocks, 4 = corner tiles (mc_set_sdf_variant)
   uint32_t* n_tris_dev;
@@ -441,7 +441,7 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
   if (!(ctx->grid_fresh && ctx->grid_pos == pos && ctx->grid_vel == vel && ctx->grid_n == n))
     build_grid(ctx, pos, vel, n, s);
   ctx->boid_state = false;
-  const NbrList* nl = ctx->force_variant == 0 ? &ctx->nbr : nullptr;
+  const NbrList* nl = ctx->force_variant != 1 ? &ctx->nbr : nullptr;
   if (n_boid > 0) {
     int rc = set_boid_params(ctx, bp);
     if (rc != SPH_OK) return rc;
@@ -459,7 +459,7 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     launch_boid_density(ctx->sc, ctx->pg, ctx->bg, n_boid, ctx->rho_bS, sb, &ctx->prof);
     if (fork) CK(cudaEventRecord(ctx->ev_join, ctx->side));
   }
-  launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, nl, s, &ctx->prof);
+  launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, nl, s, &ctx->prof, ctx->force_variant == 2);
   if (ctx->vel_pending) {  // sph_simulate_host: the velocities arrived on the upload stream while the above ran
     CK(cudaStreamWaitEvent(s, ctx->ev_up_done, 0));
     launch_gather_vel(ctx->pg, (const float4*)vel, n, s, &ctx->prof);
@@ -645,7 +645,7 @@ int sph_hashgrid_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, uint3
 
 int sph_set_force_variant(sph_ctx* ctx, int variant) {
   if (!ctx) return SPH_E_INVALID;
-  if (variant < 0 || variant > 1) return fail(ctx, SPH_E_INVALID, "force variant must be 0 or 1");
+  if (variant < 0 || variant > 2) return fail(ctx, SPH_E_INVALID, "force variant must be 0, 1 or 2");
   ctx->force_variant = variant;
   return SPH_OK;
 }

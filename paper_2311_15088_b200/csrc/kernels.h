@@ -109,7 +109,7 @@ void launch_hashgrid_count(const GridDesc& g, float h2, const float4* pos, uint3
                            uint32_t* hash_grid, uint32_t* dropped, uint32_t* ncount, cudaStream_t s, Prof* prof);
 // sph.cu
 void launch_density(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
-                    uint32_t* ncount_out, const NbrList* nl, cudaStream_t s, Prof* prof);
+                    uint32_t* ncount_out, const NbrList* nl, cudaStream_t s, Prof* prof, bool pairs = false);
 uint32_t nbr_rows();
 void launch_boid_density(const SphConst& c, const GridBuf& pg, const GridBuf& bg, uint32_t nb, float* rho_bS,
                          cudaStream_t s, Prof* prof);

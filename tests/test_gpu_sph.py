@@ -15,7 +15,7 @@ from tests.gpuutil import Sim, dev, vec_err
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(autouse=True, params=[0, 1], ids=["nbrlist", "gridwalk"])
+@pytest.fixture(autouse=True, params=[0, 1, 2], ids=["nbrlist", "gridwalk", "nbrlist-pairs"])
 def force_variant(request):
     """Every test runs on both S8 kernels: the stored-neighbour-list pass (default) and the grid walk."""
     gpuutil.FORCE_VARIANT = request.param
@@ -128,3 +128,33 @@ def test_full_size_step_matches_oracle(idx):
     with Sim(cfg) as sim:
         out = sim.step(dev(cfg["pos"]), dev(cfg["vel"]), dev(cfg["bpos"]), dev(cfg["bvel"]), cfg["boid"])
     _compare_step(cfg, out, ref, cfg["pos"])
+
+
+@pytest.mark.parametrize("case", ["config2", "sparse", "ragged"])
+def test_pair_density_is_bitwise_the_per_particle_density(case, force_variant):
+    """k_density_pairs (two targets of a cell per thread, packed binary32) performs every pair's operations in the order
+    of k_density: density, neighbour counts and the state after the step are identical bit for bit.  'sparse' has ~1
+    particle per cell (a warp's 56 slots hold more than 32 pairs: second round); 'ragged' ends inside a warp's slots."""
+    if force_variant != 2:
+        pytest.skip("compares variant 2 with variant 0 once")
+    if case == "config2":
+        cfg = W.config(2)
+        pos0, vel0 = cfg["pos"].copy(), W.uniform_box(cfg["n"], (-0.2,) * 3, (0.2,) * 3, 3, 31)
+    else:
+        cfg = W.config(1)
+        n = 4096 if case == "sparse" else 56 * 37 + 29
+        cfg = dict(cfg, n=n, n_boid=0)
+        pos0 = W.uniform_box(n, (0.0,) * 3, (1.0,) * 3, 5, 32) if case == "sparse" else cfg["pos"][:n].copy()
+        vel0 = W.uniform_box(n, (-0.2,) * 3, (0.2,) * 3, 6, 33)
+    outs = []
+    for v in (0, 2):
+        gpuutil.FORCE_VARIANT = v
+        with Sim(cfg) as sim:
+            outs.append(sim.step(dev(pos0), dev(vel0)))
+    gpuutil.FORCE_VARIANT = 2
+    for k in ("density", "ncount", "accel", "pos", "vel"):
+        assert np.array_equal(outs[0][k], outs[1][k]), k
+    ref = R.step(cfg["sph"], pos0, vel0)
+    assert np.array_equal(outs[1]["ncount"], ref["ncount"])
+    bad, worst = vec_err(outs[1]["density"], ref["density"])
+    assert bad == 0, ("density", bad, worst)
