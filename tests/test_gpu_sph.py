@@ -158,3 +158,34 @@ def test_pair_density_is_bitwise_the_per_particle_density(case, force_variant):
     assert np.array_equal(outs[1]["ncount"], ref["ncount"])
     bad, worst = vec_err(outs[1]["density"], ref["density"])
     assert bad == 0, ("density", bad, worst)
+
+
+def test_free_running_hundred_frames_config2(force_variant):
+    """BASELINE.json configs[1] as stated: 65 536 particles, 256 boids, 100 steps.  The GPU frames (sph_step + boid_step)
+    run free beside the oracle's; D:A-MULTI (ii) bounds the divergence by eps(s) = s * (1e-5 |x| + 2e-6) (2e-5 for
+    velocities).  Measured on B200 after the 100 frames: max |dpos| 2.7e-7, max |dvel| 8.7e-7, two neighbour counts off by one, so a
+    fixed bound of ten single-step floors is asserted at the end as well; the neighbour counts (integers decided on r^2 < h^2) may differ
+    only where a pair sits within rounding of h."""
+    if force_variant == 1:
+        pytest.skip("one list variant and the pair variant cover the free run; the grid walk is covered by the 10-step test")
+    cfg = W.config(2)
+    rp, rv, rbp, rbv = cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"]
+    with Sim(cfg) as sim:
+        gp, gv, gbp, gbv = dev(rp), dev(rv), dev(rbp), dev(rbv)
+        for s in range(1, 101):
+            ref = R.step(cfg["sph"], rp, rv, rbp, rbv, cfg["boid"])
+            refb = R.boid_step(cfg["sph"], cfg["boid"], rp, rv, ref["density"], rbp, rbv)
+            rp, rv, rbp, rbv = ref["pos"], ref["vel"], refb["bpos"], refb["bvel"]
+            out = sim.step(gp, gv, gbp, gbv, cfg["boid"])
+            ob = sim.boid_step(cfg["boid"], gbp, gbv)
+            if s % 10 == 0:
+                for got, want, a in ((out["pos"], rp, 2e-6), (out["vel"], rv, 2e-5), (ob["bpos"], rbp, 2e-6), (ob["bvel"], rbv, 2e-5)):
+                    bad, worst = vec_err(got[:, :3], want[:, :3], rel=1e-5 * s, abs_=a * s)
+                    assert bad == 0, (s, bad, worst)
+    assert float(np.abs(out["pos"][:, :3] - rp[:, :3]).max()) < 1e-5
+    assert float(np.abs(out["vel"][:, :3] - rv[:, :3]).max()) < 1e-4
+    assert float(np.abs(ob["bpos"][:, :3] - rbp[:, :3]).max()) < 1e-5
+    assert int((out["ncount"] != ref["ncount"]).sum()) <= cfg["n"] // 1000
+    print("free run, 100 frames: max|dpos| %.3g max|dvel| %.3g ncount mismatches %d" % (
+        float(np.abs(out["pos"][:, :3] - rp[:, :3]).max()), float(np.abs(out["vel"][:, :3] - rv[:, :3]).max()),
+        int((out["ncount"] != ref["ncount"]).sum())))
