@@ -160,19 +160,21 @@ def test_pair_density_is_bitwise_the_per_particle_density(case, force_variant):
     assert bad == 0, ("density", bad, worst)
 
 
-def test_free_running_hundred_frames_config2(force_variant):
-    """BASELINE.json configs[1] as stated: 65 536 particles, 256 boids, 100 steps.  The GPU frames (sph_step + boid_step)
-    run free beside the oracle's; D:A-MULTI (ii) bounds the divergence by eps(s) = s * (1e-5 |x| + 2e-6) (2e-5 for
-    velocities).  Measured on B200 after the 100 frames: max |dpos| 2.7e-7, max |dvel| 8.7e-7, two neighbour counts off by one, so a
-    fixed bound of ten single-step floors is asserted at the end as well; the neighbour counts (integers decided on r^2 < h^2) may differ
-    only where a pair sits within rounding of h."""
-    if force_variant == 1:
-        pytest.skip("one list variant and the pair variant cover the free run; the grid walk is covered by the 10-step test")
-    cfg = W.config(2)
+@pytest.mark.parametrize("idx,frames", [(2, 100), (3, 100), (4, 100), (5, 20)])
+def test_free_running_frames_as_baseline_states_them(idx, frames, force_variant):
+    """BASELINE.json configs[1..4] with the particle, boid and step counts they state (65 536 / 256 / 100, 262 144 / 1 024 /
+    100 with the boids pushing the fluid, 1 048 576 / 4 096 / 100, 4 194 304 / 16 384 / 20).  The GPU frames (sph_step +
+    boid_step) run free beside the oracle's; D:A-MULTI (ii) bounds the divergence by eps(s) = s * (1e-5 |x| + 2e-6) (2e-5
+    for velocities).  Measured on B200 after 100 frames of config 2: max |dpos| 2.7e-7, max |dvel| 8.7e-7, two neighbour
+    counts off by one, so a fixed bound of ten single-step floors is asserted at the end as well; the neighbour counts
+    (integers decided on r^2 < h^2) may differ only where a pair sits within rounding of h."""
+    if force_variant == 1 or (force_variant == 2 and idx != 2):
+        pytest.skip("the default list variant runs every config, the pair variant config 2; the grid walk has the 10-step test")
+    cfg = W.config(idx)
     rp, rv, rbp, rbv = cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"]
     with Sim(cfg) as sim:
         gp, gv, gbp, gbv = dev(rp), dev(rv), dev(rbp), dev(rbv)
-        for s in range(1, 101):
+        for s in range(1, frames + 1):
             ref = R.step(cfg["sph"], rp, rv, rbp, rbv, cfg["boid"])
             refb = R.boid_step(cfg["sph"], cfg["boid"], rp, rv, ref["density"], rbp, rbv)
             rp, rv, rbp, rbv = ref["pos"], ref["vel"], refb["bpos"], refb["bvel"]
@@ -186,6 +188,7 @@ def test_free_running_hundred_frames_config2(force_variant):
     assert float(np.abs(out["vel"][:, :3] - rv[:, :3]).max()) < 1e-4
     assert float(np.abs(ob["bpos"][:, :3] - rbp[:, :3]).max()) < 1e-5
     assert int((out["ncount"] != ref["ncount"]).sum()) <= cfg["n"] // 1000
-    print("free run, 100 frames: max|dpos| %.3g max|dvel| %.3g ncount mismatches %d" % (
+    print("free run, config %d, %d frames: max|dpos| %.3g max|dvel| %.3g ncount mismatches %d" % (
+        idx, frames,
         float(np.abs(out["pos"][:, :3] - rp[:, :3]).max()), float(np.abs(out["vel"][:, :3] - rv[:, :3]).max()),
         int((out["ncount"] != ref["ncount"]).sum())))
