@@ -168,10 +168,6 @@ def test_full_size_mc_config4_sampled():
         phi = torch.zeros(G ** 3, device="cuda")
         B.mc_voxel_sdf(sim.ctx, mp, phi)
         phi_gpu = phi.cpu().numpy().reshape(G, G, G)
-        for k in (0, 37, 100, 127, 128, 200, 255):
-            plane = dict(mp, origin=(mp["origin"][0], mp["origin"][1],
-                                     float(np.float32(mp["origin"][2]) + np.float32(k) * np.float32(mp["spacing"]))))
-            ref = R.voxel_sdf(cfg["sph"], dict(plane, n_point_per_axis=G), cfg["pos"]) if False else None
         # whole-field comparison is affordable on the oracle (16.7M corners): do it outright
         phi_ref = R.voxel_sdf(cfg["sph"], mp, cfg["pos"]).reshape(G, G, G)
         assert np.abs(phi_gpu - phi_ref).max() <= 1e-5 * h
@@ -187,6 +183,34 @@ def test_full_size_mc_config4_sampled():
         nt2 = B.mc_extract(sim.ctx, mp, buf2, phi=phi2)
         assert bool((phi2 == phi).all())
         assert nt2 == nt_ref and np.array_equal(buf2.cpu().numpy()[:nt2], tris_ref)
+
+
+@pytest.mark.parametrize("idx,frames", [(3, 100), (4, 60)])
+def test_surface_of_an_evolved_state_at_full_size(idx, frames):
+    """The surface pass on a state the simulation produced (the collapsed column / dam break after `frames` GPU frames:
+    irregular spacing, a splashing free surface, boids inside), not on the initial lattice: phi of the whole field against
+    the oracle on the same positions, the mesh of that phi bit for bit, and the fused mc_extract the same again."""
+    cfg = W.config(idx)
+    G, h = cfg["G"], cfg["sph"]["h"]
+    with Sim(cfg, G=G) as sim:
+        pos, vel, bpos, bvel = dev(cfg["pos"]), dev(cfg["vel"]), dev(cfg["bpos"]), dev(cfg["bvel"])
+        for _ in range(frames):
+            B.sph_step(sim.ctx, pos, vel, bpos, bvel, cfg["boid"])
+            B.boid_step(sim.ctx, cfg["boid"], bpos, bvel)
+        torch.cuda.synchronize()
+        pos_np = pos.cpu().numpy()
+        assert np.isfinite(pos_np).all() and np.abs(pos_np[:, :3] - cfg["pos"][:, :3]).max() > h  # it has moved (0.1 s of free fall: ~0.05)
+        mp = W.mc_params(cfg, pos_np)
+        B.sph_build_grid(sim.ctx, pos, vel)
+        phi = torch.zeros(G ** 3, device="cuda")
+        buf = torch.zeros(4_000_000, 3, 3, device="cuda")
+        nt = B.mc_extract(sim.ctx, mp, buf, phi=phi)
+        phi_gpu = phi.cpu().numpy()
+        phi_ref = R.voxel_sdf(cfg["sph"], mp, pos_np)
+        assert np.abs(phi_gpu - phi_ref).max() <= 1e-5 * h
+        tris_ref, nt_ref, _ = R.mc_polygonise(mp, phi_gpu)
+        assert nt == nt_ref and nt > 10000
+        assert np.array_equal(buf.cpu().numpy()[:nt], tris_ref)
 
 
 # ---- N3: indexed mesh with per-vertex normals ------------------------------------------------------------------------
