@@ -6,8 +6,10 @@ Integers (ncount, touched) bit-exact.  Floats per particle, vector norm (DESIGN.
 """
 import numpy as np
 import pytest
+import torch
 
 from oracle import refbind as R
+from paper_2311_15088_b200 import binding as B
 from paper_2311_15088_b200 import workloads as W
 from tests import gpuutil
 from tests.gpuutil import Sim, dev, vec_err
@@ -192,3 +194,33 @@ def test_free_running_frames_as_baseline_states_them(idx, frames, force_variant)
         idx, frames,
         float(np.abs(out["pos"][:, :3] - rp[:, :3]).max()), float(np.abs(out["vel"][:, :3] - rv[:, :3]).max()),
         int((out["ncount"] != ref["ncount"]).sum())))
+
+
+@pytest.mark.parametrize("idx,frames", [(2, 1000), (3, 400)])
+def test_single_step_parity_from_a_late_state(idx, frames, force_variant):
+    """Single-step parity not from the initial lattice but from a state deep into the run (config 2 after 1 s of simulated
+    time: the dam has broken, run up the far wall and fallen back -- wall clamps, compressed clusters, boids inside the
+    fluid): the GPU runs `frames` frames on its own, then one more step is compared with the oracle's step from that same
+    state with the single-step tolerances."""
+    cfg = W.config(idx)
+    with Sim(cfg) as sim:
+        pos, vel, bpos, bvel = dev(cfg["pos"]), dev(cfg["vel"]), dev(cfg["bpos"]), dev(cfg["bvel"])
+        for _ in range(frames):
+            B.sph_step(sim.ctx, pos, vel, bpos, bvel, cfg["boid"])
+            B.boid_step(sim.ctx, cfg["boid"], bpos, bvel)
+        torch.cuda.synchronize()
+        p0, v0, bp0, bv0 = (t.cpu().numpy() for t in (pos, vel, bpos, bvel))
+        assert np.isfinite(p0).all() and np.isfinite(v0).all() and np.isfinite(bp0).all() and np.isfinite(bv0).all()
+        lo, hi = np.array(cfg["sph"]["box_min"], np.float32), np.array(cfg["sph"]["box_max"], np.float32)
+        assert (p0[:, :3] >= lo).all() and (p0[:, :3] <= hi).all()
+        assert ((p0[:, :3] == lo) | (p0[:, :3] == hi)).any()  # some particles sit on a wall: the clamp is exercised
+        ref = R.step(cfg["sph"], p0, v0, bp0, bv0, cfg["boid"])
+        out = sim.step(pos, vel, bpos, bvel, cfg["boid"])
+        _compare_step(cfg, out, ref, p0)
+        assert ref["ncount"].max() > 40  # compressed regions: well above the lattice's ~30 neighbours
+        refb = R.boid_step(cfg["sph"], cfg["boid"], p0, v0, ref["density"], bp0, bv0)
+        ob = sim.boid_step(cfg["boid"], bpos, bvel)
+        bad, worst = vec_err(ob["bvel"][:, :3], refb["bvel"][:, :3], rel=2e-5, abs_=2e-6)
+        assert bad == 0, ("bvel", bad, worst)
+        bad, worst = vec_err(ob["bpos"][:, :3], refb["bpos"][:, :3])
+        assert bad == 0, ("bpos", bad, worst)
