@@ -185,7 +185,7 @@ def test_full_size_mc_config4_sampled():
         assert nt2 == nt_ref and np.array_equal(buf2.cpu().numpy()[:nt2], tris_ref)
 
 
-@pytest.mark.parametrize("idx,frames", [(3, 100), (4, 60)])
+@pytest.mark.parametrize("idx,frames", [(2, 1000), (3, 100), (3, 400), (4, 60)])
 def test_surface_of_an_evolved_state_at_full_size(idx, frames):
     """The surface pass on a state the simulation produced (the collapsed column / dam break after `frames` GPU frames:
     irregular spacing, a splashing free surface, boids inside), not on the initial lattice: phi of the whole field against
@@ -209,7 +209,7 @@ def test_surface_of_an_evolved_state_at_full_size(idx, frames):
         phi_ref = R.voxel_sdf(cfg["sph"], mp, pos_np)
         assert np.abs(phi_gpu - phi_ref).max() <= 1e-5 * h
         tris_ref, nt_ref, _ = R.mc_polygonise(mp, phi_gpu)
-        assert nt == nt_ref and nt > 10000
+        assert nt == nt_ref and nt > 1000
         assert np.array_equal(buf.cpu().numpy()[:nt], tris_ref)
 
 
