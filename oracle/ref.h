@@ -25,7 +25,9 @@
  *   boid rules ............................... pinned (hand-evaluated two-boid case, lone boid, speed cap)
  *   SPH<->boid coupling ...................... invariants only (antisymmetry, locality, brute force);
  *                                              the coupling READING is ours (D:C-COUPLE): PARITY UNPINNED
- *   voxel SDF ................................ pinned (one particle: phi = |x-x1| - rbar; symmetric pair)
+ *   voxel SDF ................................ pinned (one particle: phi = |x-x1| - rbar; symmetric pair; the weight
+ *                                              k(s) = (1-s^2)^3 of P:487: unequal pair closed form, Listing 9 written
+ *                                              out as its two loops in numpy, k -> 0 like (2 eps)^3 at the edge of R)
  *   MC table ................................. pinned (P:542 worked example edge_table[8]=0x80c, crack-free
  *                                                      faces, edge cover, orientation)
  *   indexed mesh (N3) ........................ welding pinned (expands to the triangle soup bitwise, Euler characteristic

@@ -56,6 +56,104 @@ def test_sdf_symmetric_pair_and_brute_force():
     assert (a < 0).any() and (a > 0).any()
 
 
+def _phi_at_one_corner(pts, x, R_, rbar, h=0.0625):
+    """phi of the oracle at the single point x (a 2^3 voxel grid with spacing 0: every corner is x)."""
+    mp = _mp(2, origin=tuple(float(v) for v in x), spacing=0.0, R_=R_, rbar=rbar)
+    p4 = np.zeros((len(pts), 4), np.float32)
+    p4[:, :3] = pts
+    phi = R.voxel_sdf(_sp(h), mp, p4)
+    assert np.all(phi == phi[0])
+    return float(phi[0])
+
+
+def test_sdf_weight_unequal_pair_closed_form():
+    # P:477-487 (Eq. 48-50): two particles on a line through the corner x at UNEQUAL distances d1 (towards +x) and d2
+    # (towards -x).  xbar - x = (k1 d1 - k2 d2)/(k1 + k2) along the line with k_i = (1 - d_i^2/R^2)^3, so
+    # phi = |k1 d1 - k2 d2|/(k1 + k2) - rbar.  The weights do NOT cancel here: an exponent other than 3, or k(s) taken
+    # as (1 - s)^3, moves phi by far more than the tolerance (checked below so the pin cannot go vacuous).
+    Rn, rbar = 0.0625, 0.03125
+    x = np.array([0.5, 0.5, 0.5], np.float32)
+    for d1, d2 in ((0.05, 0.02), (0.01, 0.06), (0.031, 0.047), (0.0009765625, 0.0605)):
+        pts = np.array([[0.5 + d1, 0.5, 0.5], [0.5 - d2, 0.5, 0.5]], np.float32)
+        e1 = float(np.float64(pts[0, 0]) - np.float64(x[0]))      # the distances the float32 inputs really have
+        e2 = float(np.float64(x[0]) - np.float64(pts[1, 0]))
+        k1 = (1.0 - e1 * e1 / (Rn * Rn)) ** 3
+        k2 = (1.0 - e2 * e2 / (Rn * Rn)) ** 3
+        want = abs(k1 * e1 - k2 * e2) / (k1 + k2) - rbar
+        got = _phi_at_one_corner(pts[:, :3], x, Rn, rbar)
+        assert abs(got - want) < 2e-7, (d1, d2, got, want)
+        # what plausible misreadings would give: each must be far from the closed form
+        for kk in (lambda d: (1.0 - d * d / (Rn * Rn)) ** 2,      # exponent 2
+                   lambda d: (1.0 - d / Rn) ** 3,                 # s where s^2 belongs
+                   lambda d: 1.0 - d * d / (Rn * Rn),             # exponent 1
+                   lambda d: 1.0):                                # unweighted mean
+            wrong = abs(kk(e1) * e1 - kk(e2) * e2) / (kk(e1) + kk(e2)) - rbar
+            assert abs(wrong - want) > 1e-5, (d1, d2)     # 50x the tolerance above
+
+
+def test_sdf_weight_is_listing_9_written_out():
+    # P:494-516 (Listing 9) evaluated exactly as printed, in numpy float64: loop 1 sums the kernel values
+    # (weight_divisor), loop 2 forms w_i = k_i / sum k and the weighted mean position; phi = |x - xbar| - particle_size.
+    # Also pins reading D:A-PHI (the oracle's one-pass |sum k (x_j - x)|/sum k is the two-loop form) and Eq. 50's
+    # neighbourhood (only particles with |x - x_i| < R take part).
+    rng = np.random.default_rng(5)
+    Rn, rbar = 0.0625, 0.03125
+    worst = 0.0
+    for trial in range(40):
+        npts = int(rng.integers(3, 9))
+        x = (0.3 + 0.4 * rng.random(3)).astype(np.float32)
+        d = rng.standard_normal((npts, 3))
+        d *= (rng.random((npts, 1)) * 1.25 * Rn) / np.linalg.norm(d, axis=1, keepdims=True)   # some beyond R
+        pts = (x.astype(np.float64) + d).astype(np.float32)
+        cube_corner_pos = x.astype(np.float64)
+        pp = pts.astype(np.float64)
+        neigh = [p for p in pp if np.linalg.norm(cube_corner_pos - p) < Rn * (1 - 1e-6)]
+        edge = [p for p in pp if abs(np.linalg.norm(cube_corner_pos - p) / Rn - 1) <= 1e-6]
+        if edge or not neigh:
+            continue
+        kernel = lambda s: (1.0 - s * s) ** 3                                        # noqa: E731  (P:487)
+        weight_divisor = 0.0
+        for p in neigh:
+            weight_divisor += kernel(np.linalg.norm(cube_corner_pos - p) / Rn)
+        weight_multiplier = 1.0 / weight_divisor
+        average_particle_pos = np.zeros(3)
+        for p in neigh:
+            weight_i = weight_multiplier * kernel(np.linalg.norm(cube_corner_pos - p) / Rn)
+            average_particle_pos += weight_i * p
+        want = np.linalg.norm(cube_corner_pos - average_particle_pos) - rbar
+        got = _phi_at_one_corner(pts, x, Rn, rbar)
+        worst = max(worst, abs(got - want))
+        assert len(neigh) >= 1
+    assert worst < 3e-7, worst
+
+
+def test_sdf_weight_vanishes_continuously_at_R():
+    # P:487: k(1) = 0, so a particle approaching the edge of the neighbourhood leaves the average continuously:
+    # with a fixed particle at distance a on one side and a second at distance r -> R on the other side,
+    # phi -> a - rbar, and the gap shrinks like k(r/R) ~ (2 (1 - r/R))^3 (the cube: exponent 3 and s^2 pinned again)
+    Rn, rbar, a = 0.0625, 0.03125, 0.02
+    x = np.array([0.5, 0.5, 0.5], np.float32)
+    one = _phi_at_one_corner(np.array([[0.5 + a, 0.5, 0.5]], np.float32), x, Rn, rbar)
+    gaps = []
+    for eps in (0.08, 0.04, 0.02, 0.01):
+        r = Rn * (1 - eps)
+        pts = np.array([[0.5 + a, 0.5, 0.5], [0.5 - r, 0.5, 0.5]], np.float32)
+        gaps.append(one - _phi_at_one_corner(pts, x, Rn, rbar))
+    assert all(g > 0 for g in gaps) and gaps[-1] < 2e-6
+    ratios = [gaps[i] / gaps[i + 1] for i in range(3)]
+    # halving eps divides k by ~8 (exponent 3 of a simple zero of 1 - s^2); exponent 2 would give ~4, (1 - s)^3 also 8
+    # but with k ~ eps^3 instead of (2 eps)^3: check the size too
+    assert all(6.5 < q < 9.5 for q in ratios), ratios
+    e = 0.01
+    k2 = (1 - (1 - e) ** 2) ** 3
+    k1 = (1 - (a / Rn) ** 2) ** 3
+    want_gap = (a + Rn * (1 - e)) * k2 / (k1 + k2)
+    assert abs(gaps[-1] / want_gap - 1) < 0.05
+    # beyond R the particle is no neighbour at all
+    pts = np.array([[0.5 + a, 0.5, 0.5], [0.5 - Rn * 1.001, 0.5, 0.5]], np.float32)
+    assert _phi_at_one_corner(pts, x, Rn, rbar) == one
+
+
 def test_table_worked_example_and_structure():
     tri, ntri, edge = R.mc_table()
     corners, edges = R.mc_numbering()
