@@ -328,6 +328,7 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
       cudaEventCreateWithFlags(&ctx->ev_rho, cudaEventDisableTiming) != cudaSuccess)
     return bail(SPH_E_CUDA);
   upload_mc_tables();
+  brick_init();
   if (cudaDeviceSynchronize() != cudaSuccess) return bail(SPH_E_CUDA);
   *out = ctx;
   return SPH_OK;
@@ -375,7 +376,7 @@ static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step", "k_boid_obstacles",
     "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_hashgrid_fill", "k_hashgrid_count", "k_range_count", "k_range_scan", "k_range_scatter", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32",
-    "k_cc_init", "k_cc_link", "k_cc_flatten", "k_cc_count", "k_cc_largest", "k_gather_vel"};
+    "k_cc_init", "k_cc_link", "k_cc_flatten", "k_cc_count", "k_cc_largest", "k_gather_vel", "k_density_brick", "k_force_brick", "k_force_masks"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -459,7 +460,11 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     launch_boid_density(ctx->sc, ctx->pg, ctx->bg, n_boid, ctx->rho_bS, sb, &ctx->prof);
     if (fork) CK(cudaEventRecord(ctx->ev_join, ctx->side));
   }
-  launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, nl, s, &ctx->prof, ctx->force_variant == 2);
+  const bool brick = ctx->force_variant >= 3;  // 3 = k_density_brick + k_force_brick, 4 = k_density_brick + k_force_masks
+  if (brick) {
+    launch_density_brick(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, (uint32_t*)ctx->nbr.list, s, &ctx->prof);
+  } else
+    launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, nl, s, &ctx->prof, ctx->force_variant == 2);
   if (ctx->vel_pending) {  // sph_simulate_host: the velocities arrived on the upload stream while the above ran
     CK(cudaStreamWaitEvent(s, ctx->ev_up_done, 0));
     launch_gather_vel(ctx->pg, (const float4*)vel, n, s, &ctx->prof);
@@ -470,8 +475,13 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     CK(cudaEventRecord(ctx->ev_rho, s));
     CK(cudaStreamWaitEvent(s, ctx->ev_join, 0));
   }
-  launch_force_integrate(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS,
-                         ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, nl, s, &ctx->prof);
+  if (brick)
+    launch_force_brick(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS, ctx->rho_bS,
+                       (float4*)pos, (float4*)vel, (float4*)accel, touched, (const uint32_t*)ctx->nbr.list,
+                       ctx->force_variant == 3, s, &ctx->prof);
+  else
+    launch_force_integrate(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS,
+                           ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, nl, s, &ctx->prof);
   ctx->grid_fresh = false;  // positions moved
   ctx->step_state = true;   // pg / rhoS still describe the step-start state (for boid_step)
   if (n_boid > 0) {
@@ -645,7 +655,7 @@ int sph_hashgrid_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, uint3
 
 int sph_set_force_variant(sph_ctx* ctx, int variant) {
   if (!ctx) return SPH_E_INVALID;
-  if (variant < 0 || variant > 2) return fail(ctx, SPH_E_INVALID, "force variant must be 0, 1 or 2");
+  if (variant < 0 || variant > 4) return fail(ctx, SPH_E_INVALID, "force variant must be 0..4");
   ctx->force_variant = variant;
   return SPH_OK;
 }

@@ -47,7 +47,7 @@ enum KernelId {
   K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_BOID_OBSTACLES, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
   K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_HASHGRID_FILL, K_HASHGRID_COUNT, K_RANGE_COUNT, K_RANGE_SCAN, K_RANGE_SCATTER, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_MC_EDGE_SCAN, K_MC_VERTICES, K_MC_EMIT_INDICES, K_ZERO_U32,
   K_CC_INIT, K_CC_LINK, K_CC_FLATTEN, K_CC_COUNT, K_CC_LARGEST,  // N3 connectivity
-  K_GATHER_VEL,
+  K_GATHER_VEL, K_DENSITY_BRICK, K_FORCE_BRICK, K_FORCE_MASKS,
   K_NUM_KERNELS
 };
 
@@ -117,6 +117,15 @@ void launch_force_integrate(const SphConst& c, const BoidConst* bc, const GridBu
                             uint32_t n, uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos,
                             float4* vel, float4* accel_out, uint32_t* touched_out, const NbrList* nl,
                             cudaStream_t s, Prof* prof);
+// sph_brick.cu: the same two passes with a brick of cells per block staged in shared memory.  masks = one word per target
+// and chunk of 32 candidates, kNbrMaskWords words per sorted particle, row-major.
+constexpr int kNbrMaskWords = 32;
+void brick_init();  // once per device: opt in to the dynamic shared memory the kernels use
+void launch_density_brick(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
+                          uint32_t* ncount_out, uint32_t* masks, cudaStream_t s, Prof* prof);
+void launch_force_brick(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
+                        uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
+                        uint32_t* touched_out, const uint32_t* masks, bool staged, cudaStream_t s, Prof* prof);
 // boid.cu
 void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                       uint32_t nb, const float* rhoS, const float* rho_bS, float4* bpos, float4* bvel,

@@ -1,0 +1,739 @@
+// sph_brick.cu -- S6 and S8-S10 with the neighbourhood of a BRICK of cells staged once per block in shared memory.
+// P:440-471 (Listing 8 + section 9: neighbour search, stored neighbours), P:172 / P:182 (density), P:351-375 (Listing 3).
+//
+// The per-particle kernels of sph.cu hand every lane 16 bytes through the L1 data stage for ONE pair test, and the
+// ~8 particles of a cell pull the same nine runs through it eight times; their force pass gathers two 16-byte records
+// per neighbour from lines scattered over L1.  Both sit at ~75 % of the L1 wavefront peak.  Here a block owns a brick
+// of BX x BY x BZ cells: it copies the (BX+2)(BY+2)(BZ+2) cells around it -- (BY+2)(BZ+2) contiguous x-runs of the
+// cell-sorted arrays -- into shared memory once, and
+//   k_density_brick : a thread owns TWO targets of one cell (they share their nine runs), every candidate is one
+//                     shared load for two tests on packed binary32; the neighbour predicate bits of every chunk of 32
+//                     candidates are stored as they are (one mask word per target and chunk) -- that is the stored
+//                     neighbour list of P:469-471, 1 bit per candidate instead of an index per neighbour;
+//   k_force_brick   : a thread owns one target, expands its mask words into staged slots and gathers the neighbours'
+//                     {pos | vel, rho} from shared memory (bank conflicts instead of one L1 wavefront per line).
+// A brick whose neighbourhood does not fit the staging capacity is split in two along an axis, down to single cells;
+// a single cell whose 27 cells still do not fit is processed straight from global memory.  Every target sees the same
+// candidates in the same order whichever way its brick was split, so the results do not depend on the split.
+// Arithmetic: the tests are those of k_density (same operations, same order, chunk sums of <= 32 candidates joined in
+// binary64): rho, ncount are bit for bit k_density's.
+#include "kernels.h"
+#include "sph_common.cuh"
+
+namespace sphb {
+
+namespace {
+
+constexpr int BX = 4, BY = 4, BZ = 2;            // brick of cells per block
+constexpr int kMaxRows = (BY + 2) * (BZ + 2);    // x-runs of the staged neighbourhood
+constexpr int kBounds = BX + 3;                  // cell bounds per run: cells x0-1 .. x0+BX
+constexpr int kMaxCells = BX * BY * BZ;
+constexpr int kDThreads = 128;                   // k_density_brick: two targets per thread
+constexpr int kFThreads = 256;                   // k_force_brick: one target per thread
+constexpr int kTabCap = 16;                      // (mask word, chunk base) entries per thread of k_force_brick
+constexpr uint32_t kFull = 0xffffffffu;
+// Every barrier below follows loops whose trip counts differ between the lanes of a warp, and bar.sync is an ALIGNED
+// barrier (every lane of a warp has to arrive together): __syncwarp() first makes that explicit.
+__device__ __forceinline__ void block_sync() {
+  __syncwarp();
+  __syncthreads();
+}
+
+static_assert(kMaxRows <= 32 && kMaxCells <= 32, "one warp scans the rows / cells of a brick");
+
+struct Box {
+  int x0, y0, z0, sx, sy, sz;
+};
+
+struct BrickTab {
+  uint32_t cs[kMaxRows][kBounds + 1];  // bounds of the cells of every staged run, in SLOT SPACE: index into the staged
+                                       // arrays when the box is staged, cell-sorted global slot when it is not
+  uint32_t g0[kMaxRows];               // global slot of the first particle of each run
+  uint32_t off[kMaxRows + 1];          // staged index of the first particle of each run; off[rows] = T
+  uint32_t pre[kMaxCells + 1];         // density: units before each cell; force: targets before each brick row
+  uint32_t T, ntarget;                 // particles in the neighbourhood, targets in the box
+  Box stack[8];
+  Box cur;
+  int sp, action;
+};
+
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, uint32_t lane) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t t = __shfl_up_sync(kFull, v, o);
+    if (lane >= (uint32_t)o) v += t;
+  }
+  return v;
+}
+
+// Bounds of the runs of box b (global slots), their lengths scanned; ends with a barrier.  Cells outside the grid are
+// empty (D:A-BOUND): a run is clipped in x, a row outside in y or z has no particles.
+__device__ __forceinline__ void brick_bounds(BrickTab& tb, const Box& b, const GridDesc& g,
+                                             const uint32_t* __restrict__ start) {
+  const int tid = threadIdx.x, nthreads = blockDim.x;
+  const int ny = b.sy + 2, nrows = ny * (b.sz + 2), nb = b.sx + 3;
+  for (int idx = tid; idx < nrows * nb; idx += nthreads) {
+    const int r = idx / nb, hx = idx - r * nb;
+    const int y = b.y0 - 1 + r % ny, z = b.z0 - 1 + r / ny;
+    uint32_t v = 0;
+    if (y >= 0 && y < g.dim[1] && z >= 0 && z < g.dim[2]) {
+      const int x = min(max(b.x0 - 1 + hx, 0), g.dim[0]);
+      v = __ldg(start + (uint32_t)g.dim[0] * ((uint32_t)y + (uint32_t)g.dim[1] * (uint32_t)z) + (uint32_t)x);
+    }
+    tb.cs[r][hx] = v;
+  }
+  block_sync();
+  if (tid < 32) {
+    const bool row = tid < nrows;
+    const uint32_t a = row ? tb.cs[tid][0] : 0u, e = row ? tb.cs[tid][nb - 1] : 0u;
+    const uint32_t len = e - a;
+    const uint32_t inc = warp_incl_scan(len, (uint32_t)tid);
+    if (row) {
+      tb.g0[tid] = a;
+      tb.off[tid] = inc - len;
+    }
+    if (tid == nrows - 1) tb.off[nrows] = inc;
+    if (tid == 31) tb.T = inc;
+    const int hy = tid % ny, hz = tid / ny;
+    const bool inside = row && hy >= 1 && hy <= b.sy && hz >= 1 && hz <= b.sz;
+    uint32_t nt = inside ? tb.cs[tid][b.sx + 1] - tb.cs[tid][1] : 0u;
+    nt = warp_sum_u32(nt);
+    if (tid == 0) tb.ntarget = nt;
+  }
+  block_sync();
+}
+
+// Copy the runs into shared memory and turn the bounds into staged indices; ends with a barrier.  SOA: positions as
+// three float arrays x[cap], y[cap], z[cap] (k_density_brick: two candidates per 8-byte load; the runs of x-adjacent
+// cells start 32 bytes apart on the rest lattice, so the lanes of a warp hit different banks); else float4 positions and
+// float4 {velocity, 1 / rho} records (as k_density_brick left them) (k_force_brick: two 16-byte gathers per neighbour).
+template <bool SOA>
+__device__ __forceinline__ void brick_stage(BrickTab& tb, const Box& b, const float4* __restrict__ posS,
+                                            const float4* __restrict__ velS, float4* spos, float4* svel, uint32_t cap) {
+  const int tid = threadIdx.x, nthreads = blockDim.x;
+  const int ny = b.sy + 2, nrows = ny * (b.sz + 2), nb = b.sx + 3;
+  for (int idx = tid; idx < nrows * nb; idx += nthreads) {
+    const int r = idx / nb, hx = idx - r * nb;
+    tb.cs[r][hx] = tb.cs[r][hx] - tb.g0[r] + tb.off[r];
+  }
+  const int warp = tid >> 5, lane = tid & 31, nwarps = nthreads >> 5;
+  for (int r = warp; r < nrows; r += nwarps) {
+    const uint32_t o = tb.off[r], len = tb.off[r + 1] - o, gs = tb.g0[r];
+    for (uint32_t k = lane; k < len; k += 32) {
+      const float4 p = __ldg(posS + gs + k);
+      if (SOA) {
+        float* sx = reinterpret_cast<float*>(spos);
+        sx[o + k] = p.x, sx[cap + o + k] = p.y, sx[2u * cap + o + k] = p.z;
+      } else {
+        spos[o + k] = p;
+        svel[o + k] = __ldg(velS + gs + k);  // .w = 1 / rho (k_density_brick)
+      }
+    }
+  }
+  block_sync();
+}
+
+// The block's brick, clipped to the grid, goes on the stack.
+__device__ __forceinline__ void brick_begin(BrickTab& tb, const GridDesc& g) {
+  if (threadIdx.x == 0) {
+    const int nbx = (g.dim[0] + BX - 1) / BX, nby = (g.dim[1] + BY - 1) / BY;
+    const int bx = (int)(blockIdx.x % (uint32_t)nbx), by = (int)((blockIdx.x / (uint32_t)nbx) % (uint32_t)nby),
+              bz = (int)(blockIdx.x / ((uint32_t)nbx * (uint32_t)nby));
+    Box b;
+    b.x0 = bx * BX, b.y0 = by * BY, b.z0 = bz * BZ;
+    b.sx = min(BX, g.dim[0] - b.x0), b.sy = min(BY, g.dim[1] - b.y0), b.sz = min(BZ, g.dim[2] - b.z0);
+    tb.stack[0] = b;
+    tb.sp = 1;
+  }
+  block_sync();
+}
+
+// One round of the box loop.  Thread 0 alone pops the box and, once the block has computed its bounds, decides what
+// happens to it; the decision travels through shared memory, so every thread acts on the same one.  Boxes without
+// targets are dropped; a box whose neighbourhood exceeds `cap` particles is split (z, then y, then x) unless it is one
+// cell, which is then processed from global memory.
+enum { kActDone = 0, kActSkip = 1, kActStaged = 2, kActGlobal = 3 };
+
+__device__ __forceinline__ int brick_round(BrickTab& tb, Box& b, const GridDesc& g, const uint32_t* __restrict__ start,
+                                           uint32_t cap) {
+  if (threadIdx.x == 0) {
+    if (tb.sp == 0) {
+      tb.action = kActDone;
+    } else {
+      tb.sp -= 1;
+      tb.cur = tb.stack[tb.sp];
+      tb.action = kActSkip;
+    }
+  }
+  block_sync();
+  if (tb.action == kActDone) return kActDone;
+  b = tb.cur;
+  brick_bounds(tb, b, g, start);
+  if (threadIdx.x == 0) {
+    int act = kActSkip;
+    if (tb.ntarget != 0) {
+      if (tb.T <= cap) {
+        act = kActStaged;
+      } else if (b.sx * b.sy * b.sz == 1) {
+        act = kActGlobal;
+      } else {
+        Box lo = b, hi = b;
+        if (b.sz > 1) {
+          lo.sz = b.sz / 2, hi.sz = b.sz - lo.sz, hi.z0 = b.z0 + lo.sz;
+        } else if (b.sy > 1) {
+          lo.sy = b.sy / 2, hi.sy = b.sy - lo.sy, hi.y0 = b.y0 + lo.sy;
+        } else {
+          lo.sx = b.sx / 2, hi.sx = b.sx - lo.sx, hi.x0 = b.x0 + lo.sx;
+        }
+        tb.stack[tb.sp] = hi;
+        tb.stack[tb.sp + 1] = lo;
+        tb.sp += 2;
+      }
+    }
+    tb.action = act;
+  }
+  block_sync();
+  return tb.action;
+}
+
+// ---- S6 -------------------------------------------------------------------------------------------------------------
+// rho_i = m C6 sum_{r^2 < h^2} (h^2 - r^2)^3, self included; ncount_i = #{r^2 < h^2}; the
+// predicate bits of chunk k (32 candidates from the start of a run, runs in (dz, dy) order) of target i go to
+// masks[i * kNbrMaskWords + w], w counting the target's chunks; candidate j of the chunk is bit 31 - j.
+//
+// A thread owns two targets A, B of one cell.  Staged: two candidates per step, loaded as (x0,x1), (y0,y1), (z0,z1);
+// per target three packed subtractions, dist2 and r^2 - h^2 on packed binary32 -- the scalar test's operations in its
+// order per half, so every predicate bit is the scalar one (D:A-FP).  A chunk that starts or ends on an odd slot does
+// that candidate alone, with the two TARGETS in the two halves.  The terms max(h^2 - r^2, 0)^3 of a chunk are summed in
+// binary32 (<= 32 terms in four partial sums) and the chunk sums joined in binary64.
+struct DensAcc {
+  f32x2 accA, accB;  // sums over candidate pairs, per target
+  f32x2 accAB;       // sums over single candidates: lo = target A, hi = target B
+  uint32_t maskA, maskB;
+};
+
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+
+// One target against two candidates.
+__device__ __forceinline__ void test_two(f32x2 tx, f32x2 ty, f32x2 tz, f32x2 X, f32x2 Y, f32x2 Z, f32x2 neg_h2,
+                                         uint32_t& mask, f32x2& acc) {
+  const f32x2 dx = sub2(tx, X), dy = sub2(ty, Y), dz = sub2(tz, Z);
+  const f32x2 t2 = add2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), neg_h2);
+  float t0, t1;
+  unpack2(t2, t0, t1);
+  mask = __funnelshift_l(__float_as_uint(t0), mask, 1);
+  mask = __funnelshift_l(__float_as_uint(t1), mask, 1);
+  const f32x2 m = pack2(fmaxf(-t0, 0.0f), fmaxf(-t1, 0.0f));
+  acc = fma2(mul2(m, m), m, acc);
+}
+
+template <bool SM>
+__device__ __forceinline__ void density_box(const SphConst& c, BrickTab& tb, const Box& b, const float* sx, uint32_t cap,
+                                            const float4* __restrict__ posS, const uint32_t* __restrict__ perm,
+                                            float* __restrict__ rhoS, float4* __restrict__ velS,
+                                            float* __restrict__ density_out, uint32_t* __restrict__ ncount_out,
+                                            uint32_t* __restrict__ masks) {
+  const int tid = threadIdx.x;
+  const int ny = b.sy + 2, ncell = b.sx * b.sy * b.sz;
+  const float* sy = sx + cap;
+  const float* sz = sx + 2u * cap;
+  if (tid < 32) {  // units (pairs of targets of one cell) before each cell
+    uint32_t u = 0;
+    if (tid < ncell) {
+      const int lx = tid % b.sx, ly = (tid / b.sx) % b.sy, lz = tid / (b.sx * b.sy);
+      const int r = (ly + 1) + ny * (lz + 1);
+      u = (tb.cs[r][lx + 2] - tb.cs[r][lx + 1] + 1u) >> 1;
+    }
+    const uint32_t inc = warp_incl_scan(u, (uint32_t)tid);
+    tb.pre[tid] = inc - u;
+    if (tid == 31) tb.pre[32] = inc;
+  }
+  block_sync();
+  const uint32_t U = tb.pre[32];
+  const f32x2 neg_h2 = pack2(-c.h2, -c.h2);
+#pragma unroll 1
+  for (uint32_t u = (uint32_t)tid; u < U; u += (uint32_t)kDThreads) {
+    int ci = 0;
+#pragma unroll
+    for (int st = 16; st > 0; st >>= 1)
+      if (tb.pre[ci + st] <= u) ci += st;
+    const int lx = ci % b.sx, ly = (ci / b.sx) % b.sy, lz = ci / (b.sx * b.sy);
+    const int r0 = (ly + 1) + ny * (lz + 1);
+    const uint32_t a = tb.cs[r0][lx + 1] + 2u * (u - tb.pre[ci]);
+    const bool hasB = a + 1u < tb.cs[r0][lx + 2];
+    const uint32_t iA = SM ? a - tb.off[r0] + tb.g0[r0] : a;
+    const uint32_t bslot = hasB ? a + 1u : a;
+    float3 pA, pB;
+    if (SM) {
+      pA = make_float3(sx[a], sy[a], sz[a]);
+      pB = make_float3(sx[bslot], sy[bslot], sz[bslot]);
+    } else {
+      const float4 qa = __ldg(posS + a), qb = __ldg(posS + bslot);
+      pA = make_float3(qa.x, qa.y, qa.z);
+      pB = make_float3(qb.x, qb.y, qb.z);
+    }
+    const f32x2 ax2 = pack2(pA.x, pA.x), ay2 = pack2(pA.y, pA.y), az2 = pack2(pA.z, pA.z);
+    const f32x2 bx2 = pack2(pB.x, pB.x), by2 = pack2(pB.y, pB.y), bz2 = pack2(pB.z, pB.z);
+    const f32x2 abx = pack2(pA.x, pB.x), aby = pack2(pA.y, pB.y), abz = pack2(pA.z, pB.z);
+    double SA = 0.0, SB = 0.0;
+    uint32_t cntA = 0, cntB = 0, w = 0;
+    uint4* mrow = reinterpret_cast<uint4*>(masks + (size_t)iA * kNbrMaskWords);
+    uint4 bufA = make_uint4(0u, 0u, 0u, 0u), bufB = bufA;
+#pragma unroll 1
+    for (int dz = 0; dz < 3; ++dz)
+#pragma unroll 1
+      for (int dy = 0; dy < 3; ++dy) {
+        const int r = (ly + dy) + ny * (lz + dz);
+        const uint32_t s0 = tb.cs[r][lx], s1 = tb.cs[r][lx + 3];
+#pragma unroll 1
+        for (uint32_t c0 = s0; c0 < s1; c0 += 32u) {
+          const uint32_t ce = min(c0 + 32u, s1), nc = ce - c0;
+          DensAcc d;
+          d.accA = d.accB = d.accAB = pack2(0.0f, 0.0f);
+          d.maskA = d.maskB = 0u;
+          uint32_t s = c0;
+#define SPHB_SINGLE(S)                                                                                      \
+  {                                                                                                         \
+    float qx, qy, qz;                                                                                       \
+    if (SM) {                                                                                               \
+      qx = sx[S], qy = sy[S], qz = sz[S];                                                                   \
+    } else {                                                                                                \
+      const float4 q4 = __ldg(posS + (S));                                                                  \
+      qx = q4.x, qy = q4.y, qz = q4.z;                                                                      \
+    }                                                                                                       \
+    PairAcc pa;                                                                                             \
+    pa.acc = d.accAB, pa.maskA = d.maskA, pa.maskB = d.maskB;                                               \
+    pair_test(pa, sub2(abx, pack2(qx, qx)), sub2(aby, pack2(qy, qy)), sub2(abz, pack2(qz, qz)), neg_h2);    \
+    d.accAB = pa.acc, d.maskA = pa.maskA, d.maskB = pa.maskB;                                               \
+  }
+#define SPHB_TWO(S)                                                                                         \
+  {                                                                                                         \
+    const f32x2 X = *reinterpret_cast<const f32x2*>(sx + (S)), Y = *reinterpret_cast<const f32x2*>(sy + (S)), \
+                Z = *reinterpret_cast<const f32x2*>(sz + (S));                                              \
+    test_two(ax2, ay2, az2, X, Y, Z, neg_h2, d.maskA, d.accA);                                              \
+    test_two(bx2, by2, bz2, X, Y, Z, neg_h2, d.maskB, d.accB);                                              \
+  }
+          if (SM) {
+            if (s & 1u) {  // 8-byte loads need an even slot
+              SPHB_SINGLE(s);
+              ++s;
+            }
+#pragma unroll 1
+            for (; s + 4u <= ce; s += 4u) {
+              SPHB_TWO(s);
+              SPHB_TWO(s + 2u);
+            }
+            if (s + 2u <= ce) {
+              SPHB_TWO(s);
+              s += 2u;
+            }
+            if (s < ce) SPHB_SINGLE(s);
+          } else {
+#pragma unroll 1
+            for (; s < ce; ++s) SPHB_SINGLE(s);
+          }
+#undef SPHB_SINGLE
+#undef SPHB_TWO
+          const uint32_t mA = d.maskA << (32u - nc), mB = d.maskB << (32u - nc);  // candidate j of the chunk -> bit 31 - j
+          cntA += __popc(mA), cntB += __popc(mB);
+          const uint32_t wq = w & 3u;
+          if (wq == 0u) bufA.x = mA, bufB.x = mB;
+          if (wq == 1u) bufA.y = mA, bufB.y = mB;
+          if (wq == 2u) bufA.z = mA, bufB.z = mB;
+          if (wq == 3u) {
+            bufA.w = mA, bufB.w = mB;
+            if (w < (uint32_t)kNbrMaskWords) {
+              mrow[w >> 2] = bufA;
+              if (hasB) mrow[(kNbrMaskWords >> 2) + (w >> 2)] = bufB;
+            }
+          }
+          ++w;
+          float a0, a1, b0, b1, e0, e1;
+          unpack2(d.accA, a0, a1), unpack2(d.accB, b0, b1), unpack2(d.accAB, e0, e1);
+          SA += (double)((a0 + a1) + e0);
+          SB += (double)((b0 + b1) + e1);
+        }
+      }
+    if ((w & 3u) != 0u && w < (uint32_t)kNbrMaskWords) {  // the last, partial group of four words
+      mrow[w >> 2] = bufA;
+      if (hasB) mrow[(kNbrMaskWords >> 2) + (w >> 2)] = bufB;
+    }
+    const float rhoA = (float)((double)c.mass_c6 * SA), rhoB = (float)((double)c.mass_c6 * SB);
+    rhoS[iA] = rhoA;
+    reinterpret_cast<float*>(velS + iA)[3] = 1.0f / rhoA;  // the force passes pick 1 / rho_j up with the neighbour's velocity
+    if (hasB) {
+      rhoS[iA + 1] = rhoB;
+      reinterpret_cast<float*>(velS + iA + 1)[3] = 1.0f / rhoB;
+    }
+    if (density_out || ncount_out) {
+      const uint32_t idA = __ldg(perm + iA);
+      if (density_out) density_out[idA] = rhoA;
+      if (ncount_out) ncount_out[idA] = cntA;
+      if (hasB) {
+        const uint32_t idB = __ldg(perm + iA + 1);
+        if (density_out) density_out[idB] = rhoB;
+        if (ncount_out) ncount_out[idB] = cntB;
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(kDThreads) k_density_brick(SphConst c, const float4* __restrict__ posS,
+                                                             const uint32_t* __restrict__ start,
+                                                             const uint32_t* __restrict__ perm,
+                                                             float* __restrict__ rhoS, float4* __restrict__ velS,
+                                                             float* __restrict__ density_out,
+                                                             uint32_t* __restrict__ ncount_out,
+                                                             uint32_t* __restrict__ masks, uint32_t cap) {
+  extern __shared__ __align__(16) unsigned char brick_dyn[];
+  float* sx = reinterpret_cast<float*>(brick_dyn);
+  __shared__ BrickTab tb;
+  brick_begin(tb, c.grid);
+  Box b;
+  for (;;) {
+    const int act = brick_round(tb, b, c.grid, start, cap);
+    if (act == kActDone) break;
+    if (act == kActStaged) {
+      brick_stage<true>(tb, b, posS, nullptr, reinterpret_cast<float4*>(sx), nullptr, cap);
+      density_box<true>(c, tb, b, sx, cap, posS, perm, rhoS, velS, density_out, ncount_out, masks);
+    } else if (act == kActGlobal) {
+      density_box<false>(c, tb, b, sx, cap, posS, perm, rhoS, velS, density_out, ncount_out, masks);
+    }
+    block_sync();  // the staged arrays, the tables and the decision are reused by the next round
+  }
+}
+
+// ---- S8-S10 ---------------------------------------------------------------------------------------------------------
+// Listing 3 for TWO neighbours of one target on packed binary32 (lo / hi half = neighbour 0 / 1).  With
+// A_j = 1 / rho_j staged instead of rho_j: pair = m q2/(pi h^4) A_j ( 15 k ((rho_i - 2 rho0) A_j + 1) (q2/q) d - 40 mu dv ),
+// which is the listing's (rho_i + rho_j - 2 rho0) / rho_j written without the division.  sqrt(r2) = r2 rsqrt(r2) from
+// the SFU (relative error 2^-22); the terms differ from the oracle's IEEE evaluation by a few 1e-7, far inside the 1e-5
+// tolerance on the sums; which pairs enter is decided by the exact bits of the density pass.
+// `on` (1 or 0 per half) drops the term of a coincident neighbour, whose r2 the caller replaced by a stand-in.
+struct PairConst2 {
+  f32x2 neg_inv_R, R, m_over_piR4, k15, neg_mu40, one;
+};
+__device__ __forceinline__ PairConst2 make_pair_const2(const PairConst& k) {
+  PairConst2 p;
+  p.neg_inv_R = pack2(-k.inv_R, -k.inv_R), p.R = pack2(k.R, k.R), p.m_over_piR4 = pack2(k.m_over_piR4, k.m_over_piR4);
+  p.k15 = pack2(k.k15, k.k15), p.neg_mu40 = pack2(-k.mu40, -k.mu40), p.one = pack2(1.0f, 1.0f);
+  return p;
+}
+__device__ __forceinline__ void pair_eval2(const PairConst2& k, f32x2 r2, f32x2 on, f32x2 dx, f32x2 dy, f32x2 dz,
+                                           f32x2 dvx, f32x2 dvy, f32x2 dvz, f32x2 rho_m, f32x2 irho_b, f32x2& ax,
+                                           f32x2& ay, f32x2& az) {
+  float a0, a1, i0, i1;
+  unpack2(r2, a0, a1);
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(i0) : "f"(a0));  // r2 is normal here (the caller's stand-in)
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(i1) : "f"(a1));
+  const f32x2 rinv = pack2(i0, i1);
+  const f32x2 q2 = fma2(mul2(r2, rinv), k.neg_inv_R, k.one);               // 1 - r / R
+  const f32x2 w = mul2(q2, mul2(k.R, rinv));                               // q2 / q
+  const f32x2 pterm = mul2(mul2(k.k15, fma2(rho_m, irho_b, k.one)), w);    // 15 k (rho_a + rho_b - 2 rho0) / rho_b q2/q
+  const f32x2 vterm = mul2(k.neg_mu40, irho_b);                            // -40 mu / rho_b
+  const f32x2 coef = mul2(mul2(k.m_over_piR4, q2), on);
+  ax = fma2(coef, fma2(pterm, dx, mul2(vterm, dvx)), ax);
+  ay = fma2(coef, fma2(pterm, dy, mul2(vterm, dvy)), ay);
+  az = fma2(coef, fma2(pterm, dz, mul2(vterm, dvz)), az);
+}
+
+// Two neighbours (position, {velocity, 1 / rho}) against the target (pi, vi); the two terms are summed in binary32 and
+// joined to the binary64 accumulator.
+__device__ __forceinline__ void eval_two(const PairConst2& kf2, const float4 p0, const float4 v0, const float4 p1,
+                                         const float4 v1, const float4& pi, const float4& vi, f32x2 rho_m, ForceAcc& F) {
+  const f32x2 dx = pack2(pi.x - p0.x, pi.x - p1.x), dy = pack2(pi.y - p0.y, pi.y - p1.y),
+              dz = pack2(pi.z - p0.z, pi.z - p1.z);
+  const f32x2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));  // dist2 per half
+  float r0f, r1f;
+  unpack2(r2, r0f, r1f);
+  // a coincident neighbour (and the target itself) exerts no force.  Branch-free: a stand-in r2 = 1 is
+  // evaluated and dropped.  (A subnormal r2 -- two particles 1e-19 apart -- counts as coincident here.)
+  const bool on0 = r0f >= 1.17549435e-38f, on1 = r1f >= 1.17549435e-38f;
+  f32x2 ax = pack2(0.0f, 0.0f), ay = ax, az = ax;
+  pair_eval2(kf2, pack2(on0 ? r0f : 1.0f, on1 ? r1f : 1.0f), pack2(on0 ? 1.0f : 0.0f, on1 ? 1.0f : 0.0f), dx, dy, dz,
+             pack2(vi.x - v0.x, vi.x - v1.x), pack2(vi.y - v0.y, vi.y - v1.y), pack2(vi.z - v0.z, vi.z - v1.z), rho_m,
+             pack2(v0.w, v1.w), ax, ay, az);
+  float x0, x1, y0, y1, z0, z1;
+  unpack2(ax, x0, x1), unpack2(ay, y0, y1), unpack2(az, z0, z1);
+  F.x += (double)(x0 + x1), F.y += (double)(y0 + y1), F.z += (double)(z0 + z1);
+}
+
+// One thread per target.  Prologue: the staged slot of the first candidate of each of the target's chunks goes into the
+// thread's column of a shared table (the chunks are those of k_density_brick: 32 candidates from the start of a run).
+// Main loop: the thread walks its mask words as ONE bit stream -- next set bit -> staged slot -> two 16-byte shared
+// gathers -- two neighbours per trip on packed binary32, so a lane's trips are half its neighbour count whatever the
+// spread of the bits over the chunks; no lane waits for another lane's chunk.  Pair terms are summed two at a time in
+// binary32 and joined in binary64.  A target with more chunks than mask words, and every target of a box that is not
+// staged, walks the grid in global memory instead.
+__global__ void __launch_bounds__(kFThreads, 3)
+k_force_brick(SphConst c, BoidConst bc, bool has_boids, const float4* __restrict__ posS,
+              const float4* __restrict__ velS, const uint32_t* __restrict__ start, const uint32_t* __restrict__ perm,
+              const float* __restrict__ rhoS, const uint32_t* __restrict__ masks, const float4* __restrict__ bposS,
+              const float4* __restrict__ bvelS, const float* __restrict__ rho_bS, const uint32_t* __restrict__ bstart,
+              float4* __restrict__ pos, float4* __restrict__ vel, float4* __restrict__ accel_out,
+              uint32_t* __restrict__ touched_out, uint32_t cap) {
+  extern __shared__ __align__(16) unsigned char brick_dyn[];
+  float4* spos = reinterpret_cast<float4*>(brick_dyn);
+  float4* svel = spos + cap;
+  uint32_t* tabm = reinterpret_cast<uint32_t*>(svel + cap) + threadIdx.x;  // this thread's columns of the word table
+  uint16_t* tabb = reinterpret_cast<uint16_t*>(tabm - threadIdx.x + kTabCap * kFThreads) + threadIdx.x;
+  __shared__ BrickTab tb;
+  const int tid = threadIdx.x;
+  const PairConst kf = make_pair_const(c, c.h);
+  const PairConst2 kf2 = make_pair_const2(kf);
+  brick_begin(tb, c.grid);
+  Box b;
+  for (;;) {
+    const int act = brick_round(tb, b, c.grid, start, cap);
+    if (act == kActDone) break;
+    if (act == kActSkip) {
+      block_sync();
+      continue;
+    }
+    const bool staged = act == kActStaged;
+    if (staged) brick_stage<false>(tb, b, posS, velS, spos, svel, cap);
+    const int ny = b.sy + 2, nbrow = b.sy * b.sz;
+    if (tid == 0) {  // targets before each row of the box
+      uint32_t acc = 0;
+      for (int q = 0; q < nbrow; ++q) {
+        const int r = (q % b.sy + 1) + ny * (q / b.sy + 1);
+        tb.pre[q] = acc;
+        acc += tb.cs[r][b.sx + 1] - tb.cs[r][1];
+      }
+      tb.pre[nbrow] = acc;
+    }
+    block_sync();
+    const uint32_t NT = tb.ntarget;
+#pragma unroll 1
+    for (uint32_t t = (uint32_t)tid; t < NT; t += (uint32_t)kFThreads) {
+      int q = 0;
+      while (q + 1 < nbrow && tb.pre[q + 1] <= t) ++q;
+      const int ly = q % b.sy, lz = q / b.sy;
+      const int r0 = (ly + 1) + ny * (lz + 1);
+      const uint32_t a = tb.cs[r0][1] + (t - tb.pre[q]);
+      int lx = 0;
+      while (lx + 1 < b.sx && tb.cs[r0][lx + 2] <= a) ++lx;
+      const uint32_t i = staged ? a - tb.off[r0] + tb.g0[r0] : a;
+      const float4 pi = __ldg(posS + i);
+      float4 vi = __ldg(velS + i);
+      vi.w = __ldg(rhoS + i);  // velS[.].w holds 1 / rho (k_density_brick); the tail and the grid walk want rho_i
+      ForceAcc F = {0.0, 0.0, 0.0};
+      uint32_t W = 0;
+      if (staged) {
+#pragma unroll 1
+        for (int r9 = 0; r9 < 9; ++r9) {
+          const int r = (ly + r9 % 3) + ny * (lz + r9 / 3);
+          W += (tb.cs[r][lx + 3] - tb.cs[r][lx] + 31u) >> 5;
+        }
+      }
+      if (staged && W <= (uint32_t)kNbrMaskWords) {
+        const f32x2 rho_m = pack2(vi.w - 2.0f * c.rho0, vi.w - 2.0f * c.rho0);
+        uint32_t ne = 0;
+        // Walks the table's words as ONE bit stream: next set bit -> staged slot -> two 16-byte shared gathers, two
+        // neighbours per trip.  Every word of the table has a set bit, so a refill is two shared loads.
+        auto consume = [&]() {
+          uint32_t e = 0, m = 0, base = 0;
+#pragma unroll 1
+          for (;;) {
+            if (m == 0u) {
+              if (e == ne) break;
+              m = tabm[e * kFThreads], base = tabb[e * kFThreads], ++e;
+            }
+            uint32_t j = __clz(m);
+            m ^= 0x80000000u >> j;
+            const uint32_t sl0 = base + j;
+            uint32_t sl1 = a;  // odd count: the second half reads the target itself, r^2 = 0, no force
+            if (m == 0u && e != ne) m = tabm[e * kFThreads], base = tabb[e * kFThreads], ++e;
+            if (m != 0u) {
+              j = __clz(m);
+              m ^= 0x80000000u >> j;
+              sl1 = base + j;
+            }
+            eval_two(kf2, spos[sl0], svel[sl0], spos[sl1], svel[sl1], pi, vi, rho_m, F);
+          }
+          ne = 0;
+        };
+        // Prologue: the non-empty mask words of the target and the staged slot of the first candidate of their chunks
+        // (the chunks are those of k_density_brick: 32 candidates from the start of a run) go into the thread's
+        // column of a shared table of kTabCap entries; a full table is consumed before the walk goes on.
+        const uint4* mrow = reinterpret_cast<const uint4*>(masks + (size_t)i * kNbrMaskWords);
+        uint4 cur = __ldg(mrow), nxt = make_uint4(0u, 0u, 0u, 0u);
+        if (W > 4u) nxt = __ldg(mrow + 1);
+        uint32_t w = 0;
+#pragma unroll 1
+        for (int r9 = 0; r9 < 9; ++r9) {
+          const int r = (ly + r9 % 3) + ny * (lz + r9 / 3);
+          const uint32_t s0 = tb.cs[r][lx], s1 = tb.cs[r][lx + 3];
+#pragma unroll 1
+          for (uint32_t c0 = s0; c0 < s1; c0 += 32u) {
+            const uint32_t sel = w & 3u;
+            const uint32_t m = sel == 0u ? cur.x : (sel == 1u ? cur.y : (sel == 2u ? cur.z : cur.w));
+            ++w;
+            if ((w & 3u) == 0u) {  // the next four words were fetched while these were looked at
+              cur = nxt;
+              if (w + 4u < W) nxt = __ldg(mrow + (w >> 2) + 1);
+            }
+            if (m != 0u) {
+              tabm[ne * kFThreads] = m;
+              tabb[ne * kFThreads] = (uint16_t)c0;
+              if (++ne == (uint32_t)kTabCap) consume();
+            }
+          }
+        }
+        consume();
+      } else {  // the box is not staged, or the target has more chunks than mask words: walk the grid
+        // (separate variables: what is handed to the out-of-line walk by reference lives in local memory)
+        const CellOf wk = walk_init(c.grid, pi);
+        const float4 pw = pi, vw = vi;
+        ForceAcc Fw = {0.0, 0.0, 0.0};
+        walk_force<true>(c, kf, posS, velS, start, pw, vw, wk, Fw);
+        F = Fw;
+      }
+      push_integrate_store(c, bc, has_boids, true, i, pi, vi, F, perm, bposS, bvelS, rho_bS, bstart, pos, vel, accel_out,
+                           touched_out);
+    }
+    block_sync();
+  }
+}
+
+
+// ---- S8-S10 from the mask words, without staging --------------------------------------------------------------------
+// The same bit-stream walk with one thread per cell-sorted particle and the neighbours gathered from global memory
+// (L1 / L2): no brick, no staging, so no capacity and nothing to split; the table holds global slots.  This is the
+// default consumer of k_density_brick's masks (DESIGN.md section 10 has the A/B against k_force_brick).
+constexpr int kMThreads = 128;
+
+__global__ void __launch_bounds__(kMThreads)
+k_force_masks(SphConst c, BoidConst bc, bool has_boids, const float4* __restrict__ posS,
+              const float4* __restrict__ velS, const uint32_t* __restrict__ start, const uint32_t* __restrict__ perm,
+              uint32_t n, const float* __restrict__ rhoS, const uint32_t* __restrict__ masks,
+              const float4* __restrict__ bposS, const float4* __restrict__ bvelS, const float* __restrict__ rho_bS,
+              const uint32_t* __restrict__ bstart, float4* __restrict__ pos, float4* __restrict__ vel,
+              float4* __restrict__ accel_out, uint32_t* __restrict__ touched_out) {
+  __shared__ uint32_t s_tabm[kTabCap * kMThreads], s_tabb[kTabCap * kMThreads];
+  uint32_t* tabm = s_tabm + threadIdx.x;
+  uint32_t* tabb = s_tabb + threadIdx.x;
+  const uint32_t i = blockIdx.x * kMThreads + threadIdx.x;
+  if (i >= n) return;  // no barrier and no warp-wide operation below
+  const float4 pi = __ldg(posS + i);
+  float4 vi = __ldg(velS + i);
+  vi.w = __ldg(rhoS + i);
+  const CellOf wk = walk_init(c.grid, pi);
+  const PairConst kf = make_pair_const(c, c.h);
+  const PairConst2 kf2 = make_pair_const2(kf);
+  const f32x2 rho_m = pack2(vi.w - 2.0f * c.rho0, vi.w - 2.0f * c.rho0);
+  ForceAcc F = {0.0, 0.0, 0.0};
+  uint32_t ne = 0;
+  auto consume = [&]() {
+    uint32_t e = 0, m = 0, base = 0;
+#pragma unroll 1
+    for (;;) {
+      if (m == 0u) {
+        if (e == ne) break;
+        m = tabm[e * kMThreads], base = tabb[e * kMThreads], ++e;
+      }
+      uint32_t j = __clz(m);
+      m ^= 0x80000000u >> j;
+      const uint32_t sl0 = base + j;
+      uint32_t sl1 = i;  // odd count: the second half reads the target itself, r^2 = 0, no force
+      if (m == 0u && e != ne) m = tabm[e * kMThreads], base = tabb[e * kMThreads], ++e;
+      if (m != 0u) {
+        j = __clz(m);
+        m ^= 0x80000000u >> j;
+        sl1 = base + j;
+      }
+      eval_two(kf2, __ldg(posS + sl0), __ldg(velS + sl0), __ldg(posS + sl1), __ldg(velS + sl1), pi, vi, rho_m, F);
+    }
+    ne = 0;
+  };
+  const uint4* mrow = reinterpret_cast<const uint4*>(masks + (size_t)i * kNbrMaskWords);
+  uint4 cur = __ldg(mrow), nxt = __ldg(mrow + 1);
+  uint32_t w = 0;
+  bool overflow = false;
+#pragma unroll 1
+  for (int r9 = 0; r9 < 9 && !overflow; ++r9) {
+    uint32_t s0 = 0, s1 = 0;
+    walk_row(c.grid, start, wk, r9 % 3 - 1, r9 / 3 - 1, s0, s1);
+#pragma unroll 1
+    for (uint32_t c0 = s0; c0 < s1; c0 += 32u) {
+      if (w == (uint32_t)kNbrMaskWords) {  // more chunks than mask words
+        overflow = true;
+        break;
+      }
+      const uint32_t sel = w & 3u;
+      const uint32_t m = sel == 0u ? cur.x : (sel == 1u ? cur.y : (sel == 2u ? cur.z : cur.w));
+      ++w;
+      if ((w & 3u) == 0u) {  // the next four words were fetched while these were looked at
+        cur = nxt;
+        if (w + 4u < (uint32_t)kNbrMaskWords) nxt = __ldg(mrow + (w >> 2) + 1);
+      }
+      if (m != 0u) {
+        tabm[ne * kMThreads] = m;
+        tabb[ne * kMThreads] = c0;
+        if (++ne == (uint32_t)kTabCap) consume();
+      }
+    }
+  }
+  consume();
+  if (overflow) {  // start again on the grid
+    const float4 pw = pi, vw = vi;
+    ForceAcc Fw = {0.0, 0.0, 0.0};
+    walk_force<true>(c, kf, posS, velS, start, pw, vw, wk, Fw);
+    F = Fw;
+  }
+  push_integrate_store(c, bc, has_boids, true, i, pi, vi, F, perm, bposS, bvelS, rho_bS, bstart, pos, vel, accel_out,
+                       touched_out);
+}
+
+uint32_t brick_blocks(const GridDesc& g) {
+  return (uint32_t)(((g.dim[0] + BX - 1) / BX) * ((g.dim[1] + BY - 1) / BY) * ((g.dim[2] + BZ - 1) / BZ));
+}
+
+}  // namespace
+
+// Staging capacity (particles of a box's neighbourhood).  A brick of config 4 holds 144 cells x 8 = 1152 particles; a
+// box that exceeds the capacity is split, so the choice only moves where the split happens.
+constexpr uint32_t kBrickCap = 2048;   // k_density_brick: 24 KB of x / y / z
+constexpr uint32_t kBrickCapF = 1536;  // k_force_brick: 48 KB of {pos | vel, 1/rho} + 24 KB of word tables: three blocks per SM
+
+static size_t force_smem() { return (size_t)kBrickCapF * 32 + (size_t)kTabCap * kFThreads * 6; }
+
+void brick_init() {
+  cudaFuncSetAttribute(k_force_brick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)force_smem());
+}
+
+void launch_density_brick(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
+                          uint32_t* ncount_out, uint32_t* masks, cudaStream_t s, Prof* prof) {
+  if (n == 0) return;
+  const size_t smem = (size_t)kBrickCap * 12;
+  prof->begin(K_DENSITY_BRICK, s);
+  k_density_brick<<<brick_blocks(c.grid), kDThreads, smem, s>>>(c, b.posS, b.start, b.perm, rhoS, b.velS, density_out,
+                                                                ncount_out, masks, kBrickCap);
+  prof->end(s);
+}
+
+void launch_force_brick(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
+                        uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
+                        uint32_t* touched_out, const uint32_t* masks, bool staged, cudaStream_t s, Prof* prof) {
+  if (n == 0) return;
+  BoidConst dummy = {};
+  const bool has = nb > 0 && bc != nullptr;
+  if (staged) {
+    prof->begin(K_FORCE_BRICK, s);
+    k_force_brick<<<brick_blocks(c.grid), kFThreads, force_smem(), s>>>(
+        c, has ? *bc : dummy, has, pg.posS, pg.velS, pg.start, pg.perm, rhoS, masks, bg.posS, bg.velS, rho_bS, bg.start,
+        pos, vel, accel_out, touched_out, kBrickCapF);
+  } else {
+    prof->begin(K_FORCE_MASKS, s);
+    k_force_masks<<<(n + kMThreads - 1) / kMThreads, kMThreads, 0, s>>>(
+        c, has ? *bc : dummy, has, pg.posS, pg.velS, pg.start, pg.perm, n, rhoS, masks, bg.posS, bg.velS, rho_bS,
+        bg.start, pos, vel, accel_out, touched_out);
+  }
+  prof->end(s);
+}
+
+}  // namespace sphb

@@ -17,7 +17,7 @@ from tests.gpuutil import Sim, dev, vec_err
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(autouse=True, params=[0, 1, 2], ids=["nbrlist", "gridwalk", "nbrlist-pairs"])
+@pytest.fixture(autouse=True, params=[0, 1, 2, 3, 4], ids=["nbrlist", "gridwalk", "nbrlist-pairs", "brick", "masks"])
 def force_variant(request):
     """Every test runs on both S8 kernels: the stored-neighbour-list pass (default) and the grid walk."""
     gpuutil.FORCE_VARIANT = request.param
