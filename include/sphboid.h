@@ -103,7 +103,11 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
  *   step-start fluid state retained by the sph_step of the same frame (D:C-COUPLE), edge rule, speed
  *   clamp, position update.
  * Must follow sph_step called with these same (unmodified) bpos / bvel; otherwise SPH_E_STALE_GRID.
- * Optional dv_parts[n_boid*4] float4: the sep, ali, coh, fluid velocity increments per boid. */
+ * Stream contract: bpos / bvel must not be written by anything enqueued between that sph_step and this call (the
+ * library runs this step beside the force pass of sph_step, ordered after its density pass only; work enqueued on
+ * `stream` AFTER this call sees the new boid state).
+ * Optional dv_parts[n_boid*4] float4: the sep, ali, coh, fluid velocity increments per boid; when given, the step is
+ * ordered after everything enqueued on `stream` before the call (so a fill of dv_parts on `stream` is safe). */
 int boid_step(sph_ctx* ctx, const boid_params* bp /* host */, void* bpos, void* bvel, uint32_t n_boid,
               void* stream, void* dv_parts);
 

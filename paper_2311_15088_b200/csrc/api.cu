@@ -513,7 +513,15 @@ int boid_step(sph_ctx* ctx, const boid_params* bp, void* bpos, void* bvel, uint3
   // the caller's stream then waits for it, so everything enqueued after this call still sees the new boid state
   // (with per-kernel timing on it stays on the caller's stream)
   if (!ctx->prof.on && ctx->rho_event) {
-    CK(cudaStreamWaitEvent(ctx->side, ctx->ev_rho, 0));
+    // bpos / bvel are untouched since sph_step by contract, so ordering after k_density (ev_rho) is enough for them and
+    // the kernel runs beside k_force_list.  dv_parts is a caller buffer that may have been written on `stream` just
+    // before this call (a fill): with it, the side stream is ordered after everything enqueued on `stream` so far.
+    if (dv_parts) {
+      CK(cudaEventRecord(ctx->ev_fork, s));
+      CK(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+    } else {
+      CK(cudaStreamWaitEvent(ctx->side, ctx->ev_rho, 0));
+    }
     launch_boid_step(ctx->sc, ctx->bc, ctx->pg, ctx->bg, ctx->grid_n, n_boid, ctx->rhoS, ctx->rho_bS, (float4*)bpos,
                      (float4*)bvel, (float4*)dv_parts, ctx->side, &ctx->prof);
     if (ctx->obst_normals)  // step 7 follows the position update

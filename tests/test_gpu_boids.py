@@ -26,8 +26,11 @@ def _compare(refb, out):
     assert bad == 0, ("bvel", bad, worst)
     bad, worst = vec_err(out["bpos"][:, :3], refb["bpos"][:, :3])
     assert bad == 0, ("bpos", bad, worst)
-    scale = np.abs(refb["dv_parts"]).max() + 1e-30
-    assert np.abs(out["dv_parts"] - refb["dv_parts"]).max() <= 1e-5 * scale + 1e-9
+    # the four velocity increments (sep, ali, coh, fluid) per boid and per rule, each as a vector with the per-step
+    # tolerance of DESIGN.md section 5 (1e-5 |ref| + floor); the floor is 1e-7: the increments are ~1e-3 .. 1e-1
+    for k, rule in enumerate(("sep", "ali", "coh", "fluid")):
+        bad, worst = vec_err(out["dv_parts"][:, k, :3], refb["dv_parts"][:, k, :3], abs_=1e-7)
+        assert bad == 0, ("dv_" + rule, bad, worst)
 
 
 @pytest.mark.parametrize("idx,scale", [(1, None), (2, None), (3, 2), (4, 4), (5, 4)])
@@ -128,3 +131,28 @@ def test_boid_step_with_obstacle_grid_matches_oracle(idx, scale):
         assert np.array_equal(plain["bvel"][same], out["bvel"][same])
         bad, worst = vec_err(plain["bvel"][:, :3], refb["bvel"][:, :3])
         assert bad == 0
+
+
+def test_dv_parts_written_on_the_stream_just_before_the_call_is_ordered():
+    # include/sphboid.h, boid_step stream contract: the library runs the step on a stream of its own beside the force
+    # pass; a fill of dv_parts enqueued on the caller's stream right before the call (here behind a long matmul, so it
+    # really is late) must still land BEFORE the kernel's writes
+    cfg = W.config(2)
+    ref = R.step(cfg["sph"], cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"], cfg["boid"])
+    refb = R.boid_step(cfg["sph"], cfg["boid"], cfg["pos"], cfg["vel"], ref["density"], cfg["bpos"], cfg["bvel"])
+    with Sim(cfg) as sim:
+        pos, vel, bpos, bvel = dev(cfg["pos"]), dev(cfg["vel"]), dev(cfg["bpos"]), dev(cfg["bvel"])
+        big = torch.randn(4096, 4096, device="cuda")
+        parts = torch.empty(cfg["n_boid"], 4, 4, device="cuda")
+        for _ in range(3):
+            bp, bv = bpos.clone(), bvel.clone()
+            B.sph_step(sim.ctx, pos.clone(), vel.clone(), bp, bv, cfg["boid"])
+            _ = big @ big                      # keeps the stream busy ...
+            parts.fill_(float("nan"))          # ... so this fill is still queued when boid_step is called
+            B.boid_step(sim.ctx, cfg["boid"], bp, bv, dv_parts=parts)
+            torch.cuda.synchronize()
+            got = parts.cpu().numpy()
+            assert np.isfinite(got[:, :, :3]).all()
+            for k in range(4):
+                bad, worst = vec_err(got[:, k, :3], refb["dv_parts"][:, k, :3], abs_=1e-7)
+                assert bad == 0, (k, bad, worst)
