@@ -126,6 +126,27 @@ def time_oracle(cfg, mp, min_seconds, max_frames):
     return frames, per, R.num_threads()
 
 
+def time_oracle_threads(cfg_idx, threads):
+    """Seconds per oracle frame of config `cfg_idx` with OMP_NUM_THREADS = threads (a child process: the OpenMP runtime
+    reads the variable once).  Returns (seconds, threads used) or None."""
+    code = ("import sys,time,json; sys.path.insert(0,%r)\n"
+            "import bench\n"
+            "from oracle import refbind as R\n"
+            "from paper_2311_15088_b200 import workloads as W\n"
+            "cfg=W.config(%d); mp=W.mc_params(cfg)\n"
+            "st=[cfg['pos'],cfg['vel'],cfg['bpos'],cfg['bvel']]\n"
+            "R.mc_table()\n"
+            "t=time.perf_counter(); bench.oracle_frame(R,W,cfg,mp,st); dt=time.perf_counter()-t\n"
+            "print(json.dumps([dt,R.num_threads()]))\n") % (ROOT, cfg_idx)
+    env = dict(os.environ, OMP_NUM_THREADS=str(threads))
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=300)
+        dt, used = json.loads(out.stdout.strip().splitlines()[-1])
+        return float(dt), int(used)
+    except Exception:
+        return None
+
+
 def run_reference(args, cfg_idx):
     """--impl reference: the CPU oracle as it stands, on the host cores; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -247,7 +268,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--force-variant", type=int, default=0, help="A/B: 0 = stored neighbour list (default), 1 = grid walk, 2 = list built by k_density_pairs")
+    ap.add_argument("--force-variant", type=int, default=0, help="A/B: 0 = stored neighbour list (default), 1 = grid walk, 2 = list built by k_density_pairs, 3 = brick density + brick force, 4 = brick density + mask force")
     ap.add_argument("--sdf-variant", type=int, default=0, help="A/B: 0 = cost model (default), 1-4 force one S14 kernel")
     ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (default) or the fluid cut into slabs with halo exchange (N2, SPH step only)")
@@ -382,20 +403,29 @@ def main():
     cnt_a = torch.zeros(n, dtype=torch.int32, device=fr.device)
     cnt_b = torch.zeros(n, dtype=torch.int32, device=fr.device)
     B.sph_neighbor_count(fr.ctx, fr.pos, cnt_a)
-    dropped = B.sph_hashgrid_neighbor_count(fr.ctx, fr.pos, 32, cnt_b)
+    # capacity of the unsorted grid = the largest cell population of the sorted one, so that nothing is dropped and the
+    # two searches do the same work (a comparison against a grid that drops particles would be invalid)
+    cstart = torch.zeros(C + 1, dtype=torch.int32, device=fr.device)
+    B.sph_build_grid(fr.ctx, fr.pos, None, cell_start=cstart)
+    hg_cap = int((cstart[1:] - cstart[:-1]).max().item())
+    del cstart
+    dropped = B.sph_hashgrid_neighbor_count(fr.ctx, fr.pos, hg_cap, cnt_b)
     evn = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     evn[0].record()
     for _ in range(5):
         B.sph_neighbor_count(fr.ctx, fr.pos, cnt_a)
     evn[1].record()
     for _ in range(5):
-        B.sph_hashgrid_neighbor_count(fr.ctx, fr.pos, 32, cnt_b, sync=False)
+        B.sph_hashgrid_neighbor_count(fr.ctx, fr.pos, hg_cap, cnt_b, sync=False)
     evn[2].record()
     torch.cuda.synchronize()
     nsearch = {"sorted_grid_us": 1e3 * evn[0].elapsed_time(evn[1]) / 5, "unsorted_hash_grid_us": 1e3 * evn[1].elapsed_time(evn[2]) / 5,
-               "max_per_cell": 32, "dropped": dropped, "counts_equal": bool((cnt_a == cnt_b).all().item()),
+               "max_per_cell": hg_cap, "dropped": dropped, "counts_equal": bool((cnt_a == cnt_b).all().item()),
                "what": "neighbour count of every particle: grid build + count pass (sph_neighbor_count) vs the paper's "
                        "unsorted fixed-capacity hash grid (sph_hashgrid_neighbor_count)"}
+    nsearch["valid"] = bool(nsearch["dropped"] == 0 and nsearch["counts_equal"])
+    if not nsearch["valid"]:
+        nsearch["sorted_grid_us"] = nsearch["unsorted_hash_grid_us"] = None  # not a like-for-like comparison
     del cnt_a, cnt_b
     # true neighbour pairs of that state (for the arithmetic roofline): one more SPH step with the count output
     ncount = torch.zeros(n, dtype=torch.int32, device=fr.device)
@@ -436,17 +466,9 @@ def main():
         if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else 1965.0
     pairs = RF.sdf_pairs(n, fr.mc["radius"], fr.mc["spacing"]) if RF.KERNEL_KIND.get(dominant) == "sdf" else sph_pairs
     alu = RF.alu_point(dominant, dom["avg_us"], pairs, sm_max)
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.csv")  # dram__bytes_read.sum + dram__bytes_write.sum per launch (ncu --set full)
-    if os.path.exists(tp):
-        try:
-            for row in open(tp).read().splitlines()[1:]:
-                c = row.split(",")
-                if c and c[0] == dominant:
-                    traffic = float(c[1])
-        except Exception:
-            traffic = None
-
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture; quoted only when
+    # that capture was taken on the CUDA sources this run is built from (the file is stamped with their hash), else null
+    traffic, traffic_capture, traffic_stale = RF.read_traffic(os.path.join(ROOT, "profiles", "traffic.csv"), dominant)
     hbm = {"achieved": dom["gbs"], "peak": peak, "unit": "GB/s", "frac": dom["frac"], "peak_kind": "of " + peak_kind,
            "bytes_per_launch": dom["bytes"]}
     if alu is not None:
@@ -459,6 +481,13 @@ def main():
                 "avg_us": dom["avg_us"], "share_of_step": dom["share"], "hbm": hbm}
     else:
         roof = dict(hbm, bound="hbm", kernel=dominant, traffic=traffic, avg_us=dom["avg_us"], share_of_step=dom["share"])
+    # BASELINE.json's metric is the fraction of the HBM roofline: flat keys beside the roofline that binds the kernel
+    # (algorithmic bytes of SURVEY.md 8(d) / measured time / measured HBM peak; halves from the synchronous loop)
+    roof["hbm_frac"] = dom["frac"]
+    roof["hbm_frac_sph_half"] = sim_gbs / peak
+    roof["hbm_frac_mc_half"] = mc_gbs / peak
+    roof["hbm_frac_frame"] = (sim_bytes + mc_bytes) * K / t_max / 1e9 / peak
+    roof["traffic_source"] = {"capture": traffic_capture, "stale": traffic_stale, "csrc_sha16": RF.csrc_sha16()}
 
     # ---- end to end through the C ABI with HOST buffers -------------------------------------------------
     e2e = None
@@ -493,6 +522,19 @@ def main():
         cpu = {"value": n * frames / sum(per), "unit": "particle-updates/s", "cores": cores, "kind": "oracle",
                "sample": "%d whole frame(s) of %s (%d particles, %d boids, %d^3 corners), %.1f s" %
                          (frames, cfg["name"], n, nb, G, sum(per))}
+        # single-thread beside all-core.  One frame of config 2 (65 536 particles, 64^3 corners) in
+        # a child process with OMP_NUM_THREADS=1, and the same frame with all cores for the ratio; the single-thread
+        # figure for THIS workload is that ratio applied to `value` (an extrapolation, labelled as such)
+        one, many = time_oracle_threads(2, 1), time_oracle_threads(2, cores)
+        if one and many:
+            n2 = W.config(2)["n"]
+            cpu["single_thread"] = {
+                "value": n2 / one[0], "unit": "particle-updates/s", "cores": one[1],
+                "sample": "one whole frame of config2 (%d particles), OMP_NUM_THREADS=1, %.2f s" % (n2, one[0]),
+                "all_core_same_sample": {"value": n2 / many[0], "cores": many[1], "seconds": many[0]},
+                "extrapolated_to_this_workload": {"value": cpu["value"] * many[0] / one[0],
+                                                  "how": "all-core value of this workload x (all-core / single-thread "
+                                                         "time ratio measured on config2)"}}
 
     if ranks.rank == 0:
         state_bytes = 32 * n * 2 + 16 * n + 4 * G ** 3 + 36 * n_tris + 8 * C

@@ -30,6 +30,9 @@ def kernel_bytes(n, c, nb, cb, g, t):
         # S8-S10: read posS 16, velS 16, rho 4, perm 4; write pos' 16, vel' 16
         "k_force_integrate": 72 * n,
         "k_force_list": 72 * n,     # the stored-neighbour-list variant of the same rows
+        "k_density_brick": 20 * n + 8 * c,   # S6 with a brick of cells staged per block (sph_brick.cu)
+        "k_force_brick": 72 * n,
+        "k_force_masks": 72 * n,
         # S11-S13: read bpos, bvel 32, rho_b 4, perm 4; write 32
         "k_boid_step": 72 * nb,
         # S14: write phi 4 per corner; read posS 16 per particle and the cell table 8 per cell
@@ -98,7 +101,8 @@ FLOP_PER_PAIR = {
     # three components of (pterm d - 40 mu dv) scaled and accumulated (12)
     "force": 35,
 }
-KERNEL_KIND = {"k_voxel_sdf_tiles": "sdf", "k_voxel_sdf_blocks": "sdf", "k_voxel_sdf_groups": "sdf", "k_voxel_sdf": "sdf",
+KERNEL_KIND = {"k_density_brick": "density", "k_force_brick": "force", "k_force_masks": "force",
+               "k_voxel_sdf_tiles": "sdf", "k_voxel_sdf_blocks": "sdf", "k_voxel_sdf_groups": "sdf", "k_voxel_sdf": "sdf",
                "k_density": "density", "k_force_list": "force", "k_force_integrate": "force"}
 
 
@@ -118,3 +122,43 @@ def alu_point(kernel, avg_us, pairs, sm_mhz):
     ach = flops / (avg_us * 1e-6) / 1e12
     return dict(achieved=ach, peak=peak, frac=ach / peak, flop_per_launch=flops, pairs=pairs,
                 flop_per_pair=FLOP_PER_PAIR[kind])
+
+
+def csrc_sha16():
+    """Hash of the CUDA sources the library is built from: stamps profiles/traffic.csv, so that bench.py only quotes
+    a DRAM-traffic figure captured on the code it is timing."""
+    import hashlib
+    import os
+    d = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc")
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh", ".h", ".inc")):
+            h.update(name.encode())
+            h.update(open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def read_traffic(path, kernel):
+    """profiles/traffic.csv: first line '# csrc_sha16=<hash> capture=<id>', then kernel,dram_bytes_per_launch,source.
+    Returns (bytes or None, capture id, stale?)."""
+    import os
+    if not os.path.exists(path):
+        return None, None, None
+    lines = open(path).read().splitlines()
+    sha, cap = None, None
+    if lines and lines[0].startswith("#"):
+        for tok in lines[0][1:].split():
+            if tok.startswith("csrc_sha16="):
+                sha = tok.split("=", 1)[1]
+            if tok.startswith("capture="):
+                cap = tok.split("=", 1)[1]
+    stale = sha != csrc_sha16()
+    val = None
+    for row in lines:
+        c = row.split(",")
+        if len(c) >= 2 and c[0] == kernel:
+            try:
+                val = float(c[1])
+            except ValueError:
+                val = None
+    return (None if stale else val), cap, stale
