@@ -329,6 +329,7 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
     return bail(SPH_E_CUDA);
   upload_mc_tables();
   brick_init();
+  grid_init();
   if (cudaDeviceSynchronize() != cudaSuccess) return bail(SPH_E_CUDA);
   *out = ctx;
   return SPH_OK;
@@ -376,7 +377,7 @@ static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
     "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step", "k_boid_obstacles",
     "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_hashgrid_fill", "k_hashgrid_count", "k_range_count", "k_range_scan", "k_range_scatter", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32",
-    "k_cc_init", "k_cc_link", "k_cc_flatten", "k_cc_count", "k_cc_largest", "k_gather_vel", "k_density_brick", "k_force_brick", "k_force_masks"};
+    "k_cc_init", "k_cc_link", "k_cc_flatten", "k_cc_count", "k_cc_largest", "k_gather_vel", "k_density_brick", "k_force_brick", "k_force_masks", "k_grid_small", "k_grid_small[boid grid]"};
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 

@@ -9,6 +9,7 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kScanItems = 8;                     // cells per thread in the scan
 constexpr int kScanTile = kThreads * kScanItems;  // 2048 cells per tile
+constexpr int kLongRun = 64;                      // k_reorder: runs longer than this are ranked by the whole warp
 
 // S1 + S2 (P:426-432 set_particle_count): key = hash(get_cell(p)); rank = atomicAdd(count[key], 1).
 __global__ void __launch_bounds__(kThreads) k_hash_count(GridDesc g, const float4* __restrict__ pos, uint32_t n,
@@ -162,18 +163,128 @@ __global__ void __launch_bounds__(kThreads) k_reorder(const uint32_t* __restrict
                                                       const float4* __restrict__ pos, const float4* __restrict__ vel,
                                                       uint32_t n, uint32_t* __restrict__ perm,
                                                       float4* __restrict__ posS, float4* __restrict__ velS) {
-  const uint32_t s = blockIdx.x * kThreads + threadIdx.x;
-  if (s >= n) return;
+  const uint32_t s_raw = blockIdx.x * kThreads + threadIdx.x;
+  const bool live = s_raw < n;
+  const uint32_t s = live ? s_raw : n - 1u;  // idle lanes shadow the last slot (the warp-wide part below needs them)
   const uint32_t id = __ldg(slot_id + s);
   const uint32_t c = __ldg(key + id);
   const uint32_t s0 = __ldg(start + c), s1 = __ldg(start + c + 1);
   uint32_t smaller = 0;
-  for (uint32_t t = s0; t < s1; ++t) smaller += (__ldg(slot_id + t) < id) ? 1u : 0u;
+  // A run is ~8 ids and every slot counts the smaller ids of its run on its own.  A long run (a crowded cell: the boid
+  // cluster of config 5 has ~600 boids per cell; a degenerate input has everything in one) would make that quadratic
+  // per thread, so the slots of a long run are ranked by the whole warp, one slot at a time, the lanes striding the run.
+  const bool long_run = s1 - s0 > (uint32_t)kLongRun;
+  if (!long_run)
+    for (uint32_t t = s0; t < s1; ++t) smaller += (__ldg(slot_id + t) < id) ? 1u : 0u;
+  uint32_t todo = __ballot_sync(0xffffffffu, long_run);
+  const uint32_t lane = threadIdx.x & 31u;
+  while (todo) {
+    const int src = __ffs(todo) - 1;
+    todo &= todo - 1u;
+    const uint32_t id_s = __shfl_sync(0xffffffffu, id, src), a = __shfl_sync(0xffffffffu, s0, src),
+                   e = __shfl_sync(0xffffffffu, s1, src);
+    uint32_t cnt = 0;
+    for (uint32_t t = a + lane; t < e; t += 32u) cnt += (__ldg(slot_id + t) < id_s) ? 1u : 0u;
+    cnt = warp_sum_u32(cnt);
+    if ((int)lane == src) smaller = cnt;
+  }
+  if (!live) return;
   const uint32_t dst = s0 + smaller;
   perm[dst] = id;
   posS[dst] = __ldg(pos + id);
   if (vel) velS[dst] = __ldg(vel + id);
 }
+
+// ---- S1-S5 in ONE block, for small grids (the Boid Space grid of every config; the particle grid of config 1) ---------
+// Four launches per grid build (hash + histogram, scan, scatter, reorder) are launch latency when the grid is small:
+// here one block of 1024 threads keeps the histogram / cell starts (C + 1 entries) and the arrival-ordered ids (n
+// entries), 16 bits each, in shared memory and does all four steps between block barriers.  Same results bit for bit: keys, exclusive
+// starts, canonical order (ascending id inside a cell, D:A-SORT), sorted copies, bounding box.
+constexpr int kSmallThreads = 1024;
+// counts, starts and ids all fit 16 bits (n <= 16384): (C + 2) * 2 + n * 2 bytes of shared memory.  One block zeroes,
+// scans and writes out the whole cell table through one SM, so the win over four launches ends at a few thousand cells:
+// measured on B200 with 64 000 boid cells (configs 2 and 4) the block takes 45-56 us against 33 us for the four kernels;
+// at 4 096 cells (config 1, both grids) it equals them (16 us / 9 us) with six launches fewer per frame.
+constexpr uint32_t kSmallMaxCells = 8192, kSmallMaxPoints = 16384;
+
+__global__ void __launch_bounds__(kSmallThreads) k_grid_small(GridDesc g, const float4* __restrict__ pos,
+                                                              const float4* __restrict__ vel, uint32_t n,
+                                                              uint32_t* __restrict__ key, uint32_t* __restrict__ rank,
+                                                              uint32_t* __restrict__ start, uint32_t* __restrict__ perm,
+                                                              float4* __restrict__ posS, float4* __restrict__ velS,
+                                                              uint32_t* __restrict__ aabb) {
+  extern __shared__ uint32_t s_small[];
+  __shared__ uint32_t s_scan[33];
+  __shared__ uint32_t s_box[6];
+  const uint32_t tid = threadIdx.x, C = g.C;
+  const uint32_t cell_words = (C + 2u + 1u) >> 1;                       // C + 1 entries (+ pad), two per word
+  uint16_t* s_cell = reinterpret_cast<uint16_t*>(s_small);              // histogram, then exclusive starts
+  uint16_t* s_id = reinterpret_cast<uint16_t*>(s_small + cell_words);   // [n]: ids in arrival order, slot = start + rank
+  for (uint32_t w = tid; w < cell_words; w += kSmallThreads) s_small[w] = 0u;
+  if (tid < 6) s_box[tid] = tid < 3 ? 0xffffffffu : 0u;
+  __syncthreads();
+  // S1 + S2: key, rank = arrival order in the cell (a 32-bit atomic on the word that holds the cell's
+  // 16-bit count: a count never reaches 65536, so the halves do not carry into each other); bounding box of the points
+  float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+  for (uint32_t i = tid; i < n; i += kSmallThreads) {
+    const float4 p = __ldg(pos + i);
+    const uint32_t k = cell_hash(g, cell_coord(p.x, g.lo[0], g.cell, g.dim[0]), cell_coord(p.y, g.lo[1], g.cell, g.dim[1]),
+                                 cell_coord(p.z, g.lo[2], g.cell, g.dim[2]));
+    const uint32_t sh = 16u * (k & 1u);
+    key[i] = k;
+    rank[i] = (atomicAdd(s_small + (k >> 1), 1u << sh) >> sh) & 0xffffu;
+    lo[0] = fminf(lo[0], p.x), lo[1] = fminf(lo[1], p.y), lo[2] = fminf(lo[2], p.z);
+    hi[0] = fmaxf(hi[0], p.x), hi[1] = fmaxf(hi[1], p.y), hi[2] = fmaxf(hi[2], p.z);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+      hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+    }
+  if ((tid & 31u) == 0u && tid < n) {  // a warp without a point keeps its +-3e38
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      atomicMin(s_box + a, encode_ordered(lo[a]));
+      atomicMax(s_box + 3 + a, encode_ordered(hi[a]));
+    }
+  }
+  __syncthreads();
+  if (tid < 6) aabb[tid] = s_box[tid];
+  // S3: exclusive scan of the C + 1 counts (entry C counts 0, so start[C] = n), a contiguous piece
+  // per thread
+  const uint32_t per = (C + 1u + kSmallThreads - 1u) / kSmallThreads;
+  const uint32_t c0 = min(tid * per, C + 1u), c1 = min(c0 + per, C + 1u);
+  uint32_t sum = 0;
+  for (uint32_t c = c0; c < c1; ++c) sum += s_cell[c];
+  uint32_t total;
+  uint32_t run = block_exclusive_scan(sum, s_scan, &total);
+  for (uint32_t c = c0; c < c1; ++c) {
+    const uint32_t v = s_cell[c];
+    s_cell[c] = (uint16_t)run;
+    start[c] = run;
+    run += v;
+  }
+  __syncthreads();
+  // S4a: ids in arrival order
+  for (uint32_t i = tid; i < n; i += kSmallThreads) s_id[(uint32_t)s_cell[key[i]] + rank[i]] = (uint16_t)i;
+  __syncthreads();
+  // S4b: canonical order inside a run = ascending id (D:A-SORT), with the physical copies of pos / vel
+  for (uint32_t s = tid; s < n; s += kSmallThreads) {
+    const uint32_t id = s_id[s];
+    const uint32_t c = key[id];
+    const uint32_t a = s_cell[c], e = s_cell[c + 1];
+    uint32_t smaller = 0;
+    for (uint32_t t = a; t < e; ++t) smaller += (uint32_t)s_id[t] < id ? 1u : 0u;
+    const uint32_t dst = a + smaller;
+    perm[dst] = id;
+    posS[dst] = __ldg(pos + id);
+    if (vel) velS[dst] = __ldg(vel + id);
+  }
+}
+
+static size_t small_grid_smem(uint32_t C, uint32_t n) { return (size_t)((C + 3u) >> 1) * 4 + (size_t)((n + 1u) >> 1) * 4; }
 
 // The velocity half of k_reorder on its own, for a grid that was built from the positions alone while the
 // velocities were still on their way to the device (sph_simulate_host).  velS[.].w already holds rho (k_density).
@@ -290,10 +401,23 @@ __global__ void __launch_bounds__(kThreads) k_range_scatter(const float4* __rest
 
 uint32_t grid_scan_tiles(uint32_t C) { return (C + 1 + kScanTile - 1) / kScanTile; }
 
+void grid_init() {
+  cudaFuncSetAttribute(k_grid_small, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                       (int)small_grid_smem(kSmallMaxCells, kSmallMaxPoints));
+}
+
 void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
                        ScanState& scan, cudaStream_t s, Prof* prof, bool boid_grid) {
   const uint32_t blocks = (n + kThreads - 1) / kThreads;
   const int k0 = boid_grid ? K_BOID_HASH_COUNT : K_HASH_COUNT;
+  if (n > 0 && n <= kSmallMaxPoints && g.C <= kSmallMaxCells) {  // one launch instead of four
+    prof->begin(boid_grid ? K_BOID_GRID_SMALL : K_GRID_SMALL, s);
+    k_grid_small<<<1, kSmallThreads, small_grid_smem(g.C, n), s>>>(g, pos, vel, n, b.key, b.rank, b.start, b.perm,
+                                                                    b.posS, b.velS, b.aabb);
+    prof->end(s);
+    b.aabb_now = b.aabb;
+    return;
+  }
   if (n > 0) {
     prof->begin(k0 + 0, s);
     k_hash_count<<<blocks, kThreads, 0, s>>>(g, pos, n, b.key, b.rank, b.count, b.box_part, b.aabb);

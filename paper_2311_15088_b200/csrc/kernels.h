@@ -47,7 +47,7 @@ enum KernelId {
   K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_BOID_OBSTACLES, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
   K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_HASHGRID_FILL, K_HASHGRID_COUNT, K_RANGE_COUNT, K_RANGE_SCAN, K_RANGE_SCATTER, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_MC_EDGE_SCAN, K_MC_VERTICES, K_MC_EMIT_INDICES, K_ZERO_U32,
   K_CC_INIT, K_CC_LINK, K_CC_FLATTEN, K_CC_COUNT, K_CC_LARGEST,  // N3 connectivity
-  K_GATHER_VEL, K_DENSITY_BRICK, K_FORCE_BRICK, K_FORCE_MASKS,
+  K_GATHER_VEL, K_DENSITY_BRICK, K_FORCE_BRICK, K_FORCE_MASKS, K_GRID_SMALL, K_BOID_GRID_SMALL,
   K_NUM_KERNELS
 };
 
@@ -101,6 +101,7 @@ struct SdfPlan {
 void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
                        ScanState& scan, cudaStream_t s, Prof* prof, bool boid_grid);
 uint32_t grid_scan_tiles(uint32_t C);
+void grid_init();  // once per device: opt in to the dynamic shared memory of the one-block grid build
 void launch_gather_vel(const GridBuf& b, const float4* vel, uint32_t n, cudaStream_t s, Prof* prof);
 void launch_pack_range(const float4* pos, const float4* vel, uint32_t n, int axis, float lo, float hi,
                        uint32_t* block_count, uint32_t* total_dev, float4* out_pos, float4* out_vel, uint32_t capacity,

@@ -19,6 +19,8 @@ def kernel_bytes(n, c, nb, cb, g, t):
         # S4: read key 4, pos 16, vel 16; write posS 16, velS 16, perm 4
         "k_scatter": 0,        # implementation split of S4: its bytes are counted on k_reorder
         "k_reorder": 72 * n,
+        "k_grid_small": 92 * n + 8 * c,                 # S1-S5 in one block (small grids): the four kernels' bytes
+        "k_grid_small[boid grid]": 92 * nb + 8 * cb,
         "k_hash_count[boid grid]": 20 * nb,
         "k_scan_cells[boid grid]": 8 * cb,
         "k_scatter[boid grid]": 0,
