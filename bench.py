@@ -209,12 +209,12 @@ def run_slab(args):
     cfg = W.config(args.config)
     n, K = cfg["n"], args.steps
     mc = W.mc_params(cfg)
-    lay = S.SlabLayout(cfg["sph"], ranks.world, boid=cfg["boid"], mc=mc)
+    lay = S.SlabLayout(cfg["sph"], ranks.world, boid=cfg["boid"], mc=mc, pos=cfg["pos"])  # faces cut by particle count
     p, v = S.split_initial(lay, cfg["pos"], cfg["vel"])[ranks.rank]
     bp, bv = S.split_initial(lay, cfg["bpos"], cfg["bvel"])[ranks.rank]
     be = S.GpuBackend(cfg["sph"], min(n, 2 * (n // ranks.world) + (1 << 16)), device=dev, boid_capacity=cfg["n_boid"],
                       mc_points=mc["n_point_per_axis"])
-    ex = (S.DistExchange(ranks.dist, ranks.rank, ranks.world, torch.device("cuda", dev)) if ranks.world > 1
+    ex = (S.DistExchange(ranks.dist, ranks.rank, ranks.world, torch.device("cuda", dev), capacity=max(1 << 16, n // 4)) if ranks.world > 1
           else S.LoopbackExchange(1))
     sim = S.SlabSim(lay, ranks.rank, be, ex, be.to_device(p), be.to_device(v), be.to_device(bp), be.to_device(bv),
                     cfg["boid"])

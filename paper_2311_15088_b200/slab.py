@@ -44,7 +44,10 @@ import numpy as np
 class SlabLayout:
     """Which rank owns which x-range (pure host logic, no device)."""
 
-    def __init__(self, sph, world, axis=None, boid=None, mc=None):
+    def __init__(self, sph, world, axis=None, boid=None, mc=None, pos=None):
+        """pos (optional, (n, >=3) host array): cut the faces by PARTICLE count instead of uniformly in cells -- the
+        cell-column histogram along the slab axis (what the grid build's start[] prefix gives on the device) is cut
+        into `world` pieces of near-equal population, still at cell boundaries and never narrower than a halo."""
         lo, hi = np.asarray(sph["box_min"], np.float64), np.asarray(sph["box_max"], np.float64)
         self.h = float(sph["h"])
         self.axis = int(np.argmax(hi - lo)) if axis is None else int(axis)
@@ -59,12 +62,39 @@ class SlabLayout:
         self.mc = mc
         if mc is not None:
             self.fluid_halo = max(self.fluid_halo, float(mc["radius"]) + float(mc["spacing"]))
-        if self.world > 1 and self.cells_per_rank * self.h < max(self.fluid_halo, self.boid_halo):
-            raise ValueError("slabs must be at least one halo wide (ghosts come from the two neighbours only)")
         self.origin = float(np.float32(lo[self.axis]))
+        min_cells = int(math.ceil(max(self.fluid_halo, self.boid_halo) / self.h - 1e-9))
+        if pos is None:
+            cuts = [self.cells_per_rank * r for r in range(1, self.world)]
+        else:
+            x = np.asarray(pos)[:, self.axis].astype(np.float32)
+            col = np.clip(np.floor((x - np.float32(self.origin)) / np.float32(self.h)).astype(np.int64), 0, self.dim - 1)
+            cuts = self.balanced_cuts(np.bincount(col, minlength=self.dim), self.world, min_cells)
+        widths = np.diff([0] + list(cuts) + [self.dim])
+        if self.world > 1 and (len(cuts) != self.world - 1 or (widths < min_cells).any()):
+            raise ValueError("slabs must be at least one halo wide (ghosts come from the two neighbours only)")
+        self.cuts = [int(c) for c in cuts]
         # faces in binary32, the precision positions are compared in
-        self.faces = [float(np.float32(self.origin + np.float32(self.cells_per_rank * r) * np.float32(self.h)))
-                      for r in range(1, self.world)]
+        self.faces = [float(np.float32(self.origin + np.float32(c) * np.float32(self.h))) for c in self.cuts]
+
+    @staticmethod
+    def balanced_cuts(hist, world, min_cells):
+        """Cell indices of the world - 1 faces: face r goes where the running particle count reaches r / world of the
+        total, moved as little as needed so that every slab (the outermost ones too) is >= min_cells cells wide."""
+        hist = np.asarray(hist, np.int64)
+        dim = hist.shape[0]
+        cum = np.concatenate([[0], np.cumsum(hist)])
+        total = int(cum[-1])
+        cuts = []
+        for r in range(1, world):
+            c = int(np.searchsorted(cum, total * r / world, side="left"))
+            # the nearer of the two cell boundaries around the target count
+            if c > 0 and abs(cum[c - 1] - total * r / world) <= abs(cum[min(c, dim)] - total * r / world):
+                c -= 1
+            lo = (cuts[-1] if cuts else 0) + min_cells
+            hi = dim - (world - r) * min_cells
+            cuts.append(min(max(c, lo), hi))
+        return cuts
 
     def bounds(self, rank):
         """[lo, hi) of rank's slab; the outermost slabs are open."""
@@ -114,53 +144,56 @@ class LoopbackExchange:
 
 
 class DistExchange:
-    """torch.distributed neighbour exchange (NCCL on GPUs, gloo on CPU tensors): counts first, then the payloads."""
+    """torch.distributed neighbour exchange (NCCL on GPUs, gloo on CPU tensors).  Count and payload travel in ONE
+    message per neighbour and direction: a preallocated buffer of capacity + 1 rows of 8 floats, row 0 carrying the
+    row count (as a binary32 integer, exact below 2^24), rows 1.. the (pos | vel) records.  The message size is fixed,
+    so nothing has to be known before the receive is posted: one batch of sends / receives per exchange and one host
+    read of the two received counts, no count round trip and no allocation per step.  The tensors `collect` returns are
+    views of the receive buffers: valid until the next collect (SlabSim copies them into [owned | ghosts] at once)."""
 
-    def __init__(self, dist, rank, world, device):
+    def __init__(self, dist, rank, world, device, capacity=1 << 18):
+        import torch
         self.dist, self.rank, self.world, self.device = dist, rank, world, device
+        self.capacity = int(capacity)
         self.pending = {}
+        mk = lambda: torch.zeros(self.capacity + 1, 8, dtype=torch.float32, device=device)  # noqa: E731
+        self.send = {"l": mk(), "r": mk()}
+        self.recv = {"l": mk(), "r": mk()}
+        self.counts = torch.zeros(2, dtype=torch.float32, device=device)
 
     def post(self, rank, tag, to_left, to_right):
         self.pending[tag] = (to_left, to_right)
 
+    def _fill(self, side, t):
+        buf = self.send[side]
+        k = 0 if t is None else int(t[0].shape[0])
+        if k > self.capacity:
+            raise RuntimeError("exchange buffer too small: %d rows > capacity %d" % (k, self.capacity))
+        buf[0, 0] = float(k)
+        if k:
+            buf[1:1 + k, 0:4] = t[0]
+            buf[1:1 + k, 4:8] = t[1]
+        return buf
+
     def collect(self, rank, tag):
-        import torch
         to_left, to_right = self.pending.pop(tag)
         dist = self.dist
         left, right = rank - 1, rank + 1
         has_l, has_r = rank > 0, rank < self.world - 1
-
-        def count(t):
-            return torch.tensor([0 if t is None else t[0].shape[0]], dtype=torch.int64, device=self.device)
-
-        n_from = {"l": torch.zeros(1, dtype=torch.int64, device=self.device),
-                  "r": torch.zeros(1, dtype=torch.int64, device=self.device)}
         ops = []
         if has_l:
-            ops += [dist.P2POp(dist.isend, count(to_left), left), dist.P2POp(dist.irecv, n_from["l"], left)]
+            ops += [dist.P2POp(dist.isend, self._fill("l", to_left), left), dist.P2POp(dist.irecv, self.recv["l"], left)]
         if has_r:
-            ops += [dist.P2POp(dist.isend, count(to_right), right), dist.P2POp(dist.irecv, n_from["r"], right)]
+            ops += [dist.P2POp(dist.isend, self._fill("r", to_right), right), dist.P2POp(dist.irecv, self.recv["r"], right)]
         for w in (dist.batch_isend_irecv(ops) if ops else []):
             w.wait()
-        nl, nr = int(n_from["l"].item()), int(n_from["r"].item())
-        like = to_left if to_left is not None else to_right
-        dtype = like[0].dtype if like is not None else torch.float32
-        recv_l = (torch.empty(nl, 4, dtype=dtype, device=self.device), torch.empty(nl, 4, dtype=dtype, device=self.device))
-        recv_r = (torch.empty(nr, 4, dtype=dtype, device=self.device), torch.empty(nr, 4, dtype=dtype, device=self.device))
-        ops = []
-        if has_l:
-            if to_left is not None and to_left[0].shape[0]:
-                ops += [dist.P2POp(dist.isend, to_left[0].contiguous(), left), dist.P2POp(dist.isend, to_left[1].contiguous(), left)]
-            if nl:
-                ops += [dist.P2POp(dist.irecv, recv_l[0], left), dist.P2POp(dist.irecv, recv_l[1], left)]
-        if has_r:
-            if to_right is not None and to_right[0].shape[0]:
-                ops += [dist.P2POp(dist.isend, to_right[0].contiguous(), right), dist.P2POp(dist.isend, to_right[1].contiguous(), right)]
-            if nr:
-                ops += [dist.P2POp(dist.irecv, recv_r[0], right), dist.P2POp(dist.irecv, recv_r[1], right)]
-        for w in (dist.batch_isend_irecv(ops) if ops else []):
-            w.wait()
-        return (recv_l if nl else None), (recv_r if nr else None)
+        self.counts[0] = self.recv["l"][0, 0] if has_l else 0.0
+        self.counts[1] = self.recv["r"][0, 0] if has_r else 0.0
+        nl, nr = (int(v) for v in self.counts.tolist())  # the one host read of this exchange
+        out = []
+        for side, k in (("l", nl), ("r", nr)):
+            out.append((self.recv[side][1:1 + k, 0:4], self.recv[side][1:1 + k, 4:8]) if k else None)
+        return out[0], out[1]
 
 
 class GpuBackend:

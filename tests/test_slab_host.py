@@ -232,3 +232,29 @@ def test_decomposed_step_under_gloo_world_size_2(tmp_path):
         parts.append((a[:, :4], a[:, 4:]))
     gp, gv = gather_by_id(parts, cfg["n"])
     assert np.abs(gp[:, :3] - rp[:, :3]).max() <= 1e-6 and np.abs(gv[:, :3] - rv[:, :3]).max() <= 1e-5
+
+
+def test_faces_cut_by_particle_count_balance_config4_over_8_ranks():
+    """N2: config 4's fluid fills half of the box along the slab axis, so uniform cell slabs leave half of the ranks
+    empty at t = 0 (max owned / mean = 2.0); faces cut from the cell-column histogram balance it within 10 %, stay on
+    cell boundaries, keep every slab at least a halo wide, and every coordinate still has exactly one owner."""
+    cfg = W.config(4)
+    mc = W.mc_params(cfg)
+    for world in (2, 4, 8):
+        uni = S.SlabLayout(cfg["sph"], world, boid=cfg["boid"], mc=mc)
+        bal = S.SlabLayout(cfg["sph"], world, boid=cfg["boid"], mc=mc, pos=cfg["pos"])
+        x = cfg["pos"][:, bal.axis]
+        own_u = np.bincount(uni.owner(x), minlength=world)
+        own_b = np.bincount(bal.owner(x), minlength=world)
+        assert own_u.sum() == own_b.sum() == cfg["n"]
+        assert own_u.max() / (cfg["n"] / world) > 1.9
+        assert own_b.max() / (cfg["n"] / world) <= 1.10
+        widths = np.diff([0] + bal.cuts + [bal.dim])
+        assert (widths * bal.h >= max(bal.fluid_halo, bal.boid_halo) - 1e-9).all()
+        for r in range(world):
+            lo, hi = bal.bounds(r)
+            sel = bal.owner(x) == r
+            assert ((x[sel] >= np.float32(lo)) & (x[sel] < np.float32(hi))).all()
+    # a histogram with everything in one column cannot be balanced: the cuts fall back to the narrowest legal slabs
+    cuts = S.SlabLayout.balanced_cuts(np.array([0, 0, 1000, 0, 0, 0, 0, 0, 0, 0, 0, 0]), 3, 3)
+    assert cuts == [3, 6] or (np.diff([0] + cuts + [12]) >= 3).all()
