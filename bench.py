@@ -268,8 +268,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--force-variant", type=int, default=0, help="A/B: 0 = stored neighbour list (default), 1 = grid walk, 2 = list built by k_density_pairs, 3 = brick density + brick force, 4 = brick density + mask force")
-    ap.add_argument("--sdf-variant", type=int, default=0, help="A/B: 0 = cost model (default), 1-4 force one S14 kernel")
+    ap.add_argument("--force-variant", type=int, default=0, help="A/B: 0 = stored neighbour list (default), 1 = brick density pass + neighbour masks")
+    ap.add_argument("--sdf-variant", type=int, default=0, help="A/B: 0 = cost model (default), 1 = per-corner walk, 2 = corner tiles")
     ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (default) or the fluid cut into slabs with halo exchange (N2, SPH step only)")
     args = ap.parse_args()

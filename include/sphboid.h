@@ -34,8 +34,7 @@ typedef enum {
   SPH_E_INVALID = -1,    /* null / misaligned pointer, n > max, h <= 0, empty box, bad params */
   SPH_E_CAPACITY = -2,   /* triangle buffer too small: nothing past capacity written, count still returned */
   SPH_E_STALE_GRID = -3, /* call needs a grid / step state that is not current */
-  SPH_E_CUDA = -4,       /* CUDA runtime error, see sph_last_error */
-  SPH_E_UNIMPL = -5
+  SPH_E_CUDA = -4        /* CUDA runtime error, see sph_last_error */
 } sph_status;
 
 /* SPH parameters.  bound = {min,max} and cell size d (Eq. 47); h, rho0, k, mu
@@ -144,11 +143,12 @@ int sph_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, void* stream, 
 int sph_hashgrid_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, uint32_t max_per_cell, void* stream,
                                 uint32_t* ncount, uint32_t* dropped_host);
 
-/* S8 has two kernels that compute the same forces: 0 (default) = the density pass stores each
- * particle's neighbour list (the paper's section 9 design) and the force pass reads it; 1 = the force pass
- * walks the 27 cells again; 2 = as 0, with the list and the densities produced by k_density_pairs (two particles of a
- * cell per thread; same results bit for bit, measured A/B in DESIGN.md section 10).  Tests and A/B measurements force
- * one.  Any other value: SPH_E_INVALID. */
+/* S6 / S8 exist twice, computing the same densities and forces (DESIGN.md sections 6 and 10): 0 (default) = the density
+ * pass stores each particle's neighbour list as 16-bit entries (the paper's section 9 design) and the force
+ * pass reads it; 1 = the density pass stages a brick of cells per block in shared memory and stores the neighbour
+ * predicate as one bit per candidate, the force pass walks those bits.  Measured on B200: equal at ~8 particles per
+ * cell (config 4), 1 is 9 % faster per frame at ~15 per cell (config 5).  Host-side setting, takes effect with the next
+ * sph_step.  Any other value: SPH_E_INVALID. */
 int sph_set_force_variant(sph_ctx* ctx, int variant);
 
 /* S14: voxel signed distance phi(x) = |x - xbar| - rbar, xbar the kernel-weighted mean neighbour position
@@ -166,10 +166,9 @@ int mc_voxel_sdf(sph_ctx* ctx, const mc_params* mp /* host */, void* stream, flo
  * buffer keeps its old contents.  Host-side setting, takes effect with the next call. */
 int mc_set_cube_range(sph_ctx* ctx, int axis, uint32_t lo, uint32_t hi);
 
-/* S14 has four kernels that compute the same phi: 1 = one thread per corner, 2 = a warp per
- * group of particle cells, 3 = a warp per block of 4x4x2 corners with a filtered candidate list, 4 = a warp per tile
- * of 8x8x4 corners, 2x2x2 corners per lane, with per-lane candidate lists.  0 (default) picks by a cost model from the
- * voxel spacing; the others force one (tests, A/B measurements). */
+/* S14 has two kernels that compute the same phi: 1 = one thread per corner (coarse voxel grids),
+ * 2 = a warp per tile of 8x8x4 corners, 2x2x2 corners per lane, with per-lane candidate lists (fine grids).  0 (default)
+ * picks by a cost model from the voxel spacing; the others force one (tests, A/B measurements). */
 int mc_set_sdf_variant(sph_ctx* ctx, int variant);
 
 /* S15-S17: marching cubes on a given phi[G^3] (Listing 10-11, Eq. 51): case per cube,

@@ -11,7 +11,7 @@ _f = C.c_float
 _u32 = C.c_uint32
 _vp = C.c_void_p
 
-SPH_OK, SPH_E_INVALID, SPH_E_CAPACITY, SPH_E_STALE_GRID, SPH_E_CUDA, SPH_E_UNIMPL = 0, -1, -2, -3, -4, -5
+SPH_OK, SPH_E_INVALID, SPH_E_CAPACITY, SPH_E_STALE_GRID, SPH_E_CUDA = 0, -1, -2, -3, -4
 
 
 class SphParams(C.Structure):

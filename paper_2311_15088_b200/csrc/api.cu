@@ -23,12 +23,10 @@ struct sph_ctx {
   float* rho_bS;
   float* phi;   // [Gmax^3]
   uint32_t* mc_bits;  // [ceil(Gmax/32) * Gmax^2] corner sign bits of the surface pass
-  uint32_t* sdf_first;  // corner partition tables of the surface pass (SdfPlan::first)
-  uint32_t sdf_first_cap;
   NbrList nbr;           // stored neighbour list of the last sph_step
-  int force_variant;     // 0 = stored neighbour list (k_force_list), 1 = grid walk (k_force_integrate), 2 = list built by k_density_pairs
+  int force_variant;     // 0 = stored neighbour list (k_density + k_force_list), 1 = neighbour masks (k_density_brick + k_force_masks)
   uint32_t cube_lo[3], cube_hi[3];  // mc_set_cube_range: cubes the polygoniser handles (default: all)
-  int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = cell groups, 3 = corner blocks, 4 = corner tiles (mc_set_sdf_variant)
+  int sdf_variant;       // 0 = cost model, 1 = per-corner, 2 = corner tiles (mc_set_sdf_variant)
   uint32_t* n_tris_dev;
   uint32_t* mc_prefix;   // [words of mc_bits] vertex-id prefix of the indexed mesh (N3)
   uint32_t* n_verts_dev;
@@ -288,9 +286,7 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
       cudaMalloc(&ctx->mc_prefix, std::max<size_t>(mc_bits_words((uint32_t)G), 1) * 4) != cudaSuccess || cudaMalloc(&ctx->mc_nwork, 8) != cudaSuccess ||
       cudaMalloc(&ctx->mc_work, std::max<size_t>(mc_num_segments((uint32_t)G), 1) * 8) != cudaSuccess || cudaMalloc(&ctx->nbr.cnt, nn * 2) != cudaSuccess ||
       cudaMalloc(&ctx->nbr.list, (size_t)nbr_rows() * (ctx->nbr.stride = (uint32_t)((nn + 63) & ~(size_t)63)) * 2) != cudaSuccess ||
-      cudaMalloc(&ctx->sdf_first, (size_t)(ctx->sdf_first_cap = (uint32_t)(sc.grid.dim[0] + sc.grid.dim[1] +
-                                                                          sc.grid.dim[2] + 3 * (2 * 16 + 3))) * 4) !=
-          cudaSuccess || cudaMalloc(&ctx->scan.ticket, 4) != cudaSuccess ||
+      cudaMalloc(&ctx->scan.ticket, 4) != cudaSuccess ||
       cudaMalloc(&ctx->scan.ctl, 8) != cudaSuccess)
     return bail(SPH_E_CUDA);
   ctx->max_tiles = std::max(std::max(grid_scan_tiles(sc.grid.C), grid_scan_tiles(ctx->boid_cells_cap)),
@@ -328,7 +324,6 @@ int sph_create(sph_ctx** out, const sph_params* p, int device) {
       cudaEventCreateWithFlags(&ctx->ev_rho, cudaEventDisableTiming) != cudaSuccess)
     return bail(SPH_E_CUDA);
   upload_mc_tables();
-  brick_init();
   grid_init();
   if (cudaDeviceSynchronize() != cudaSuccess) return bail(SPH_E_CUDA);
   *out = ctx;
@@ -340,7 +335,7 @@ int sph_destroy(sph_ctx* ctx) {
   cudaSetDevice(ctx->device);
   free_grid(ctx->pg);
   free_grid(ctx->bg);
-  cudaFree(ctx->nbr.list), cudaFree(ctx->nbr.cnt), cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->n_verts_dev), cudaFree(ctx->mc_prefix), cudaFree(ctx->mc_work), cudaFree(ctx->mc_nwork), cudaFree(ctx->sdf_first);
+  cudaFree(ctx->nbr.list), cudaFree(ctx->nbr.cnt), cudaFree(ctx->rhoS), cudaFree(ctx->rho_bS), cudaFree(ctx->phi), cudaFree(ctx->mc_bits), cudaFree(ctx->n_tris_dev), cudaFree(ctx->n_verts_dev), cudaFree(ctx->mc_prefix), cudaFree(ctx->mc_work), cudaFree(ctx->mc_nwork);
   cudaFree(ctx->scan.status), cudaFree(ctx->scan.ticket), cudaFree(ctx->scan_mc.status), cudaFree(ctx->scan_mc.ticket), cudaFree(ctx->scan.ctl), cudaFree(ctx->scan_mc.ctl);
   sph_profile_enable(ctx, 0);
   free(ctx->prof.recs);
@@ -375,9 +370,12 @@ uint64_t sph_launch_count(const sph_ctx* ctx) { return ctx ? ctx->prof.launches 
 
 static const char* const kKernelNames[K_NUM_KERNELS] = {
     "k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]", "k_scan_cells[boid grid]",
-    "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density", "k_boid_density", "k_force_integrate", "k_force_list", "k_boid_step", "k_boid_obstacles",
-    "k_voxel_sdf", "k_sdf_axis_tables", "k_voxel_sdf_groups", "k_voxel_sdf_blocks", "k_voxel_sdf_tiles", "k_hashgrid_fill", "k_hashgrid_count", "k_range_count", "k_range_scan", "k_range_scatter", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices", "k_mc_emit_indices", "k_zero_u32",
-    "k_cc_init", "k_cc_link", "k_cc_flatten", "k_cc_count", "k_cc_largest", "k_gather_vel", "k_density_brick", "k_force_brick", "k_force_masks", "k_grid_small", "k_grid_small[boid grid]"};
+    "k_scatter[boid grid]", "k_reorder[boid grid]", "k_grid_small", "k_grid_small[boid grid]", "k_gather_vel",
+    "k_density", "k_density_brick", "k_boid_density", "k_force_list", "k_force_masks", "k_boid_step", "k_boid_obstacles",
+    "k_voxel_sdf", "k_voxel_sdf_tiles", "k_mc_signs", "k_mc_count", "k_mc_emit", "k_mc_edge_scan", "k_mc_vertices",
+    "k_mc_emit_indices", "k_zero_u32", "k_cc_init", "k_cc_link", "k_cc_flatten", "k_cc_count", "k_cc_largest",
+    "k_hashgrid_fill", "k_hashgrid_count", "k_range_count", "k_range_scan", "k_range_scatter"};
+
 
 const char* sph_kernel_name(uint32_t kernel_id) { return kernel_id < K_NUM_KERNELS ? kKernelNames[kernel_id] : nullptr; }
 
@@ -443,7 +441,7 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
   if (!(ctx->grid_fresh && ctx->grid_pos == pos && ctx->grid_vel == vel && ctx->grid_n == n))
     build_grid(ctx, pos, vel, n, s);
   ctx->boid_state = false;
-  const NbrList* nl = ctx->force_variant != 1 ? &ctx->nbr : nullptr;
+  const bool brick = ctx->force_variant == 1;
   if (n_boid > 0) {
     int rc = set_boid_params(ctx, bp);
     if (rc != SPH_OK) return rc;
@@ -461,11 +459,10 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     launch_boid_density(ctx->sc, ctx->pg, ctx->bg, n_boid, ctx->rho_bS, sb, &ctx->prof);
     if (fork) CK(cudaEventRecord(ctx->ev_join, ctx->side));
   }
-  const bool brick = ctx->force_variant >= 3;  // 3 = k_density_brick + k_force_brick, 4 = k_density_brick + k_force_masks
-  if (brick) {
+  if (brick)
     launch_density_brick(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, (uint32_t*)ctx->nbr.list, s, &ctx->prof);
-  } else
-    launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, nl, s, &ctx->prof, ctx->force_variant == 2);
+  else
+    launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, &ctx->nbr, s, &ctx->prof);
   if (ctx->vel_pending) {  // sph_simulate_host: the velocities arrived on the upload stream while the above ran
     CK(cudaStreamWaitEvent(s, ctx->ev_up_done, 0));
     launch_gather_vel(ctx->pg, (const float4*)vel, n, s, &ctx->prof);
@@ -477,12 +474,11 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     CK(cudaStreamWaitEvent(s, ctx->ev_join, 0));
   }
   if (brick)
-    launch_force_brick(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS, ctx->rho_bS,
-                       (float4*)pos, (float4*)vel, (float4*)accel, touched, (const uint32_t*)ctx->nbr.list,
-                       ctx->force_variant == 3, s, &ctx->prof);
+    launch_force_masks(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS, ctx->rho_bS,
+                       (float4*)pos, (float4*)vel, (float4*)accel, touched, (const uint32_t*)ctx->nbr.list, s, &ctx->prof);
   else
-    launch_force_integrate(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS,
-                           ctx->rho_bS, (float4*)pos, (float4*)vel, (float4*)accel, touched, nl, s, &ctx->prof);
+    launch_force_list(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rho_bS, (float4*)pos,
+                      (float4*)vel, (float4*)accel, touched, ctx->nbr, s, &ctx->prof);
   ctx->grid_fresh = false;  // positions moved
   ctx->step_state = true;   // pg / rhoS still describe the step-start state (for boid_step)
   if (n_boid > 0) {
@@ -551,7 +547,7 @@ static int voxel_sdf(sph_ctx* ctx, const mc_params* mp, void* stream, float* phi
   if (!phi) return fail(ctx, SPH_E_INVALID, "phi is NULL");
   if (!ctx->grid_fresh) return fail(ctx, SPH_E_STALE_GRID, "mc needs sph_build_grid on the current positions");
   CK(cudaSetDevice(ctx->device));
-  ctx->bits_ready = launch_voxel_sdf(ctx->sc, m, ctx->pg, ctx->sdf_first, ctx->sdf_first_cap, phi,
+  ctx->bits_ready = launch_voxel_sdf(ctx->sc, m, ctx->pg, phi,
                                      want_bits ? ctx->mc_bits : nullptr, ctx->sdf_variant, (cudaStream_t)stream,
                                      &ctx->prof);
   CK(cudaGetLastError());
@@ -591,7 +587,7 @@ int mc_set_cube_range(sph_ctx* ctx, int axis, uint32_t lo, uint32_t hi) {
 
 int mc_set_sdf_variant(sph_ctx* ctx, int variant) {
   if (!ctx) return SPH_E_INVALID;
-  if (variant < 0 || variant > 4) return fail(ctx, SPH_E_INVALID, "sdf variant must be 0..4");
+  if (variant < 0 || variant > 2) return fail(ctx, SPH_E_INVALID, "sdf variant must be 0, 1 or 2");
   ctx->sdf_variant = variant;
   return SPH_OK;
 }
@@ -664,7 +660,7 @@ int sph_hashgrid_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, uint3
 
 int sph_set_force_variant(sph_ctx* ctx, int variant) {
   if (!ctx) return SPH_E_INVALID;
-  if (variant < 0 || variant > 4) return fail(ctx, SPH_E_INVALID, "force variant must be 0..4");
+  if (variant < 0 || variant > 1) return fail(ctx, SPH_E_INVALID, "force variant must be 0 or 1");
   ctx->force_variant = variant;
   return SPH_OK;
 }

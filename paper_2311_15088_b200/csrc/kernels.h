@@ -44,12 +44,14 @@ struct McConst {
 enum KernelId {
   K_HASH_COUNT = 0, K_SCAN_CELLS, K_SCATTER, K_REORDER,          // particle grid
   K_BOID_HASH_COUNT, K_BOID_SCAN_CELLS, K_BOID_SCATTER, K_BOID_REORDER,  // same kernels on the Boid Space grid
-  K_DENSITY, K_BOID_DENSITY, K_FORCE_INTEGRATE, K_FORCE_LIST, K_BOID_STEP, K_BOID_OBSTACLES, K_VOXEL_SDF, K_SDF_AXIS_TABLES, K_VOXEL_SDF_GROUPS,
-  K_VOXEL_SDF_BLOCKS, K_VOXEL_SDF_TILES, K_HASHGRID_FILL, K_HASHGRID_COUNT, K_RANGE_COUNT, K_RANGE_SCAN, K_RANGE_SCATTER, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_MC_EDGE_SCAN, K_MC_VERTICES, K_MC_EMIT_INDICES, K_ZERO_U32,
-  K_CC_INIT, K_CC_LINK, K_CC_FLATTEN, K_CC_COUNT, K_CC_LARGEST,  // N3 connectivity
-  K_GATHER_VEL, K_DENSITY_BRICK, K_FORCE_BRICK, K_FORCE_MASKS, K_GRID_SMALL, K_BOID_GRID_SMALL,
+  K_GRID_SMALL, K_BOID_GRID_SMALL, K_GATHER_VEL,
+  K_DENSITY, K_DENSITY_BRICK, K_BOID_DENSITY, K_FORCE_LIST, K_FORCE_MASKS, K_BOID_STEP, K_BOID_OBSTACLES,
+  K_VOXEL_SDF, K_VOXEL_SDF_TILES, K_MC_SIGNS, K_MC_COUNT, K_MC_EMIT, K_MC_EDGE_SCAN, K_MC_VERTICES, K_MC_EMIT_INDICES,
+  K_ZERO_U32, K_CC_INIT, K_CC_LINK, K_CC_FLATTEN, K_CC_COUNT, K_CC_LARGEST,  // N3 connectivity
+  K_HASHGRID_FILL, K_HASHGRID_COUNT, K_RANGE_COUNT, K_RANGE_SCAN, K_RANGE_SCATTER,
   K_NUM_KERNELS
 };
+
 
 // Launch bookkeeping: a counter always; when `on`, a CUDA event before and after every launch, recorded on
 // the launching stream (the kernels of one call are serialised on that stream anyway).
@@ -89,14 +91,6 @@ struct NbrList {
   uint32_t stride;      // elements between rows, a multiple of 64
 };
 
-// Corner partition of the voxel grid by particle cell (mc.cu, k_voxel_sdf_groups).
-struct SdfPlan {
-  int nv[3];            // virtual cells per axis: dim + 2 reach + 2
-  int gsz[3];           // group size in virtual cells
-  int ng[3];            // groups per axis
-  uint32_t* first[3];   // [nv+1] first corner index of each virtual cell
-};
-
 // grid.cu
 void launch_build_grid(const GridDesc& g, GridBuf& b, const float4* pos, const float4* vel, uint32_t n,
                        ScanState& scan, cudaStream_t s, Prof* prof, bool boid_grid);
@@ -110,23 +104,21 @@ void launch_hashgrid_count(const GridDesc& g, float h2, const float4* pos, uint3
                            uint32_t* hash_grid, uint32_t* dropped, uint32_t* ncount, cudaStream_t s, Prof* prof);
 // sph.cu
 void launch_density(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
-                    uint32_t* ncount_out, const NbrList* nl, cudaStream_t s, Prof* prof, bool pairs = false);
+                    uint32_t* ncount_out, const NbrList* nl, cudaStream_t s, Prof* prof);
 uint32_t nbr_rows();
 void launch_boid_density(const SphConst& c, const GridBuf& pg, const GridBuf& bg, uint32_t nb, float* rho_bS,
                          cudaStream_t s, Prof* prof);
-void launch_force_integrate(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg,
-                            uint32_t n, uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos,
-                            float4* vel, float4* accel_out, uint32_t* touched_out, const NbrList* nl,
-                            cudaStream_t s, Prof* prof);
-// sph_brick.cu: the same two passes with a brick of cells per block staged in shared memory.  masks = one word per target
-// and chunk of 32 candidates, kNbrMaskWords words per sorted particle, row-major.
+void launch_force_list(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
+                       uint32_t nb, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
+                       uint32_t* touched_out, const NbrList& nl, cudaStream_t s, Prof* prof);
+// sph_brick.cu: S6 with a brick of cells per block staged in shared memory, S8-S10 from the masks it stores.  masks = one
+// word per target and chunk of 32 candidates, kNbrMaskWords words per sorted particle, row-major.
 constexpr int kNbrMaskWords = 32;
-void brick_init();  // once per device: opt in to the dynamic shared memory the kernels use
 void launch_density_brick(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
                           uint32_t* ncount_out, uint32_t* masks, cudaStream_t s, Prof* prof);
-void launch_force_brick(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
+void launch_force_masks(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                         uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
-                        uint32_t* touched_out, const uint32_t* masks, bool staged, cudaStream_t s, Prof* prof);
+                        uint32_t* touched_out, const uint32_t* masks, cudaStream_t s, Prof* prof);
 // boid.cu
 void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                       uint32_t nb, const float* rhoS, const float* rho_bS, float4* bpos, float4* bvel,
@@ -136,9 +128,9 @@ void launch_boid_obstacles(const ObstacleConst& oc, const float4* normals, const
 // mc.cu
 void upload_mc_tables();
 void mc_table_host(int8_t* tri, uint8_t* ntri);
-bool launch_voxel_sdf(const SphConst& c, const McConst& m, const GridBuf& pg, uint32_t* sdf_first,
-                      uint32_t sdf_first_cap, float* phi, uint32_t* sign_bits /* optional */, int variant,
-                      cudaStream_t s, Prof* prof);  // true if it also filled the corner sign bit field
+bool launch_voxel_sdf(const SphConst& c, const McConst& m, const GridBuf& pg, float* phi,
+                      uint32_t* sign_bits /* optional */, int variant, cudaStream_t s,
+                      Prof* prof);  // true if it also filled the corner sign bit field
 void launch_mc_polygonise(const McConst& m, const float* phi, uint32_t* bits, bool bits_ready, float* tris,
                           uint32_t capacity, uint32_t* n_tris_dev, uint2* work, uint32_t* n_work, ScanState& scan,
                           cudaStream_t s, Prof* prof);

@@ -1,22 +1,19 @@
-// sph_brick.cu -- S6 and S8-S10 with the neighbourhood of a BRICK of cells staged once per block in shared memory.
-// P:440-471 (Listing 8 + section 9: neighbour search, stored neighbours), P:172 / P:182 (density), P:351-375 (Listing 3).
+// sph_brick.cu -- S6 with the neighbourhood of a BRICK of cells staged once per block in shared memory, and S8-S10 from
+// the neighbour masks it stores.  P:440-471 (Listing 8 + section 9: neighbour search, stored neighbours), P:172 / P:182
+// (density), P:351-375 (Listing 3).  Selected by sph_set_force_variant(ctx, 1); DESIGN.md section 10 has the A/B.
 //
-// The per-particle kernels of sph.cu hand every lane 16 bytes through the L1 data stage for ONE pair test, and the
-// ~8 particles of a cell pull the same nine runs through it eight times; their force pass gathers two 16-byte records
-// per neighbour from lines scattered over L1.  Both sit at ~75 % of the L1 wavefront peak.  Here a block owns a brick
-// of BX x BY x BZ cells: it copies the (BX+2)(BY+2)(BZ+2) cells around it -- (BY+2)(BZ+2) contiguous x-runs of the
-// cell-sorted arrays -- into shared memory once, and
-//   k_density_brick : a thread owns TWO targets of one cell (they share their nine runs), every candidate is one
-//                     shared load for two tests on packed binary32; the neighbour predicate bits of every chunk of 32
-//                     candidates are stored as they are (one mask word per target and chunk) -- that is the stored
-//                     neighbour list of P:469-471, 1 bit per candidate instead of an index per neighbour;
-//   k_force_brick   : a thread owns one target, expands its mask words into staged slots and gathers the neighbours'
-//                     {pos | vel, rho} from shared memory (bank conflicts instead of one L1 wavefront per line).
+//   k_density_brick : a block owns a brick of BX x BY x BZ cells and copies the (BX+2)(BY+2)(BZ+2) cells around it --
+//                     (BY+2)(BZ+2) contiguous x-runs of the cell-sorted positions -- into shared memory once.  A thread
+//                     owns TWO targets of one cell (they share their nine runs) and tests two candidates per step on
+//                     packed binary32.  The neighbour predicate bits of every chunk of 32 candidates are stored as they
+//                     are (one mask word per target and chunk): the stored neighbour list of P:469-471 at 1 bit per
+//                     candidate instead of an index per neighbour.
+//   k_force_masks   : one thread per particle walks its mask words as one bit stream and gathers the neighbours.
 // A brick whose neighbourhood does not fit the staging capacity is split in two along an axis, down to single cells;
 // a single cell whose 27 cells still do not fit is processed straight from global memory.  Every target sees the same
-// candidates in the same order whichever way its brick was split, so the results do not depend on the split.
-// Arithmetic: the tests are those of k_density (same operations, same order, chunk sums of <= 32 candidates joined in
-// binary64): rho, ncount are bit for bit k_density's.
+// candidates in the same chunks whichever way its brick was split, so the masks do not depend on the split.
+// Arithmetic: every predicate bit is decided by the operations of D:A-FP in their order (per half of a packed
+// instruction); the density terms of a chunk are summed in binary32 and the chunk sums joined in binary64.
 #include "kernels.h"
 #include "sph_common.cuh"
 
@@ -29,8 +26,7 @@ constexpr int kMaxRows = (BY + 2) * (BZ + 2);    // x-runs of the staged neighbo
 constexpr int kBounds = BX + 3;                  // cell bounds per run: cells x0-1 .. x0+BX
 constexpr int kMaxCells = BX * BY * BZ;
 constexpr int kDThreads = 128;                   // k_density_brick: two targets per thread
-constexpr int kFThreads = 256;                   // k_force_brick: one target per thread
-constexpr int kTabCap = 16;                      // (mask word, chunk base) entries per thread of k_force_brick
+constexpr int kTabCap = 16;                      // (mask word, chunk base) entries per thread of k_force_masks
 constexpr uint32_t kFull = 0xffffffffu;
 // Every barrier below follows loops whose trip counts differ between the lanes of a warp, and bar.sync is an ALIGNED
 // barrier (every lane of a warp has to arrive together): __syncwarp() first makes that explicit.
@@ -103,13 +99,12 @@ __device__ __forceinline__ void brick_bounds(BrickTab& tb, const Box& b, const G
   block_sync();
 }
 
-// Copy the runs into shared memory and turn the bounds into staged indices; ends with a barrier.  SOA: positions as
-// three float arrays x[cap], y[cap], z[cap] (k_density_brick: two candidates per 8-byte load; the runs of x-adjacent
-// cells start 32 bytes apart on the rest lattice, so the lanes of a warp hit different banks); else float4 positions and
-// float4 {velocity, 1 / rho} records (as k_density_brick left them) (k_force_brick: two 16-byte gathers per neighbour).
-template <bool SOA>
-__device__ __forceinline__ void brick_stage(BrickTab& tb, const Box& b, const float4* __restrict__ posS,
-                                            const float4* __restrict__ velS, float4* spos, float4* svel, uint32_t cap) {
+// Copy the runs into shared memory and turn the bounds into staged indices; ends with a barrier.  Positions are staged
+// as three float arrays x[cap], y[cap], z[cap]: two candidates per 8-byte load, and the runs of x-adjacent cells start
+// 32 bytes apart on the rest lattice, so the lanes of a warp hit different banks (with float4 records they start 128
+// bytes apart -- the same banks -- and every candidate load was a two-way conflict).
+__device__ __forceinline__ void brick_stage(BrickTab& tb, const Box& b, const float4* __restrict__ posS, float* sx,
+                                            uint32_t cap) {
   const int tid = threadIdx.x, nthreads = blockDim.x;
   const int ny = b.sy + 2, nrows = ny * (b.sz + 2), nb = b.sx + 3;
   for (int idx = tid; idx < nrows * nb; idx += nthreads) {
@@ -121,13 +116,7 @@ __device__ __forceinline__ void brick_stage(BrickTab& tb, const Box& b, const fl
     const uint32_t o = tb.off[r], len = tb.off[r + 1] - o, gs = tb.g0[r];
     for (uint32_t k = lane; k < len; k += 32) {
       const float4 p = __ldg(posS + gs + k);
-      if (SOA) {
-        float* sx = reinterpret_cast<float*>(spos);
-        sx[o + k] = p.x, sx[cap + o + k] = p.y, sx[2u * cap + o + k] = p.z;
-      } else {
-        spos[o + k] = p;
-        svel[o + k] = __ldg(velS + gs + k);  // .w = 1 / rho (k_density_brick)
-      }
+      sx[o + k] = p.x, sx[cap + o + k] = p.y, sx[2u * cap + o + k] = p.z;
     }
   }
   block_sync();
@@ -398,7 +387,7 @@ __global__ void __launch_bounds__(kDThreads) k_density_brick(SphConst c, const f
     const int act = brick_round(tb, b, c.grid, start, cap);
     if (act == kActDone) break;
     if (act == kActStaged) {
-      brick_stage<true>(tb, b, posS, nullptr, reinterpret_cast<float4*>(sx), nullptr, cap);
+      brick_stage(tb, b, posS, sx, cap);
       density_box<true>(c, tb, b, sx, cap, posS, perm, rhoS, velS, density_out, ncount_out, masks);
     } else if (act == kActGlobal) {
       density_box<false>(c, tb, b, sx, cap, posS, perm, rhoS, velS, density_out, ncount_out, masks);
@@ -462,149 +451,16 @@ __device__ __forceinline__ void eval_two(const PairConst2& kf2, const float4 p0,
   F.x += (double)(x0 + x1), F.y += (double)(y0 + y1), F.z += (double)(z0 + z1);
 }
 
-// One thread per target.  Prologue: the staged slot of the first candidate of each of the target's chunks goes into the
-// thread's column of a shared table (the chunks are those of k_density_brick: 32 candidates from the start of a run).
-// Main loop: the thread walks its mask words as ONE bit stream -- next set bit -> staged slot -> two 16-byte shared
-// gathers -- two neighbours per trip on packed binary32, so a lane's trips are half its neighbour count whatever the
-// spread of the bits over the chunks; no lane waits for another lane's chunk.  Pair terms are summed two at a time in
-// binary32 and joined in binary64.  A target with more chunks than mask words, and every target of a box that is not
-// staged, walks the grid in global memory instead.
-__global__ void __launch_bounds__(kFThreads, 3)
-k_force_brick(SphConst c, BoidConst bc, bool has_boids, const float4* __restrict__ posS,
-              const float4* __restrict__ velS, const uint32_t* __restrict__ start, const uint32_t* __restrict__ perm,
-              const float* __restrict__ rhoS, const uint32_t* __restrict__ masks, const float4* __restrict__ bposS,
-              const float4* __restrict__ bvelS, const float* __restrict__ rho_bS, const uint32_t* __restrict__ bstart,
-              float4* __restrict__ pos, float4* __restrict__ vel, float4* __restrict__ accel_out,
-              uint32_t* __restrict__ touched_out, uint32_t cap) {
-  extern __shared__ __align__(16) unsigned char brick_dyn[];
-  float4* spos = reinterpret_cast<float4*>(brick_dyn);
-  float4* svel = spos + cap;
-  uint32_t* tabm = reinterpret_cast<uint32_t*>(svel + cap) + threadIdx.x;  // this thread's columns of the word table
-  uint16_t* tabb = reinterpret_cast<uint16_t*>(tabm - threadIdx.x + kTabCap * kFThreads) + threadIdx.x;
-  __shared__ BrickTab tb;
-  const int tid = threadIdx.x;
-  const PairConst kf = make_pair_const(c, c.h);
-  const PairConst2 kf2 = make_pair_const2(kf);
-  brick_begin(tb, c.grid);
-  Box b;
-  for (;;) {
-    const int act = brick_round(tb, b, c.grid, start, cap);
-    if (act == kActDone) break;
-    if (act == kActSkip) {
-      block_sync();
-      continue;
-    }
-    const bool staged = act == kActStaged;
-    if (staged) brick_stage<false>(tb, b, posS, velS, spos, svel, cap);
-    const int ny = b.sy + 2, nbrow = b.sy * b.sz;
-    if (tid == 0) {  // targets before each row of the box
-      uint32_t acc = 0;
-      for (int q = 0; q < nbrow; ++q) {
-        const int r = (q % b.sy + 1) + ny * (q / b.sy + 1);
-        tb.pre[q] = acc;
-        acc += tb.cs[r][b.sx + 1] - tb.cs[r][1];
-      }
-      tb.pre[nbrow] = acc;
-    }
-    block_sync();
-    const uint32_t NT = tb.ntarget;
-#pragma unroll 1
-    for (uint32_t t = (uint32_t)tid; t < NT; t += (uint32_t)kFThreads) {
-      int q = 0;
-      while (q + 1 < nbrow && tb.pre[q + 1] <= t) ++q;
-      const int ly = q % b.sy, lz = q / b.sy;
-      const int r0 = (ly + 1) + ny * (lz + 1);
-      const uint32_t a = tb.cs[r0][1] + (t - tb.pre[q]);
-      int lx = 0;
-      while (lx + 1 < b.sx && tb.cs[r0][lx + 2] <= a) ++lx;
-      const uint32_t i = staged ? a - tb.off[r0] + tb.g0[r0] : a;
-      const float4 pi = __ldg(posS + i);
-      float4 vi = __ldg(velS + i);
-      vi.w = __ldg(rhoS + i);  // velS[.].w holds 1 / rho (k_density_brick); the tail and the grid walk want rho_i
-      ForceAcc F = {0.0, 0.0, 0.0};
-      uint32_t W = 0;
-      if (staged) {
-#pragma unroll 1
-        for (int r9 = 0; r9 < 9; ++r9) {
-          const int r = (ly + r9 % 3) + ny * (lz + r9 / 3);
-          W += (tb.cs[r][lx + 3] - tb.cs[r][lx] + 31u) >> 5;
-        }
-      }
-      if (staged && W <= (uint32_t)kNbrMaskWords) {
-        const f32x2 rho_m = pack2(vi.w - 2.0f * c.rho0, vi.w - 2.0f * c.rho0);
-        uint32_t ne = 0;
-        // Walks the table's words as ONE bit stream: next set bit -> staged slot -> two 16-byte shared gathers, two
-        // neighbours per trip.  Every word of the table has a set bit, so a refill is two shared loads.
-        auto consume = [&]() {
-          uint32_t e = 0, m = 0, base = 0;
-#pragma unroll 1
-          for (;;) {
-            if (m == 0u) {
-              if (e == ne) break;
-              m = tabm[e * kFThreads], base = tabb[e * kFThreads], ++e;
-            }
-            uint32_t j = __clz(m);
-            m ^= 0x80000000u >> j;
-            const uint32_t sl0 = base + j;
-            uint32_t sl1 = a;  // odd count: the second half reads the target itself, r^2 = 0, no force
-            if (m == 0u && e != ne) m = tabm[e * kFThreads], base = tabb[e * kFThreads], ++e;
-            if (m != 0u) {
-              j = __clz(m);
-              m ^= 0x80000000u >> j;
-              sl1 = base + j;
-            }
-            eval_two(kf2, spos[sl0], svel[sl0], spos[sl1], svel[sl1], pi, vi, rho_m, F);
-          }
-          ne = 0;
-        };
-        // Prologue: the non-empty mask words of the target and the staged slot of the first candidate of their chunks
-        // (the chunks are those of k_density_brick: 32 candidates from the start of a run) go into the thread's
-        // column of a shared table of kTabCap entries; a full table is consumed before the walk goes on.
-        const uint4* mrow = reinterpret_cast<const uint4*>(masks + (size_t)i * kNbrMaskWords);
-        uint4 cur = __ldg(mrow), nxt = make_uint4(0u, 0u, 0u, 0u);
-        if (W > 4u) nxt = __ldg(mrow + 1);
-        uint32_t w = 0;
-#pragma unroll 1
-        for (int r9 = 0; r9 < 9; ++r9) {
-          const int r = (ly + r9 % 3) + ny * (lz + r9 / 3);
-          const uint32_t s0 = tb.cs[r][lx], s1 = tb.cs[r][lx + 3];
-#pragma unroll 1
-          for (uint32_t c0 = s0; c0 < s1; c0 += 32u) {
-            const uint32_t sel = w & 3u;
-            const uint32_t m = sel == 0u ? cur.x : (sel == 1u ? cur.y : (sel == 2u ? cur.z : cur.w));
-            ++w;
-            if ((w & 3u) == 0u) {  // the next four words were fetched while these were looked at
-              cur = nxt;
-              if (w + 4u < W) nxt = __ldg(mrow + (w >> 2) + 1);
-            }
-            if (m != 0u) {
-              tabm[ne * kFThreads] = m;
-              tabb[ne * kFThreads] = (uint16_t)c0;
-              if (++ne == (uint32_t)kTabCap) consume();
-            }
-          }
-        }
-        consume();
-      } else {  // the box is not staged, or the target has more chunks than mask words: walk the grid
-        // (separate variables: what is handed to the out-of-line walk by reference lives in local memory)
-        const CellOf wk = walk_init(c.grid, pi);
-        const float4 pw = pi, vw = vi;
-        ForceAcc Fw = {0.0, 0.0, 0.0};
-        walk_force<true>(c, kf, posS, velS, start, pw, vw, wk, Fw);
-        F = Fw;
-      }
-      push_integrate_store(c, bc, has_boids, true, i, pi, vi, F, perm, bposS, bvelS, rho_bS, bstart, pos, vel, accel_out,
-                           touched_out);
-    }
-    block_sync();
-  }
-}
-
-
-// ---- S8-S10 from the mask words, without staging --------------------------------------------------------------------
-// The same bit-stream walk with one thread per cell-sorted particle and the neighbours gathered from global memory
-// (L1 / L2): no brick, no staging, so no capacity and nothing to split; the table holds global slots.  This is the
-// default consumer of k_density_brick's masks (DESIGN.md section 10 has the A/B against k_force_brick).
+// ---- S8-S10 from the mask words ------------------------------------------------------------------------------------
+// One thread per cell-sorted particle.  Prologue: the non-empty mask words of the particle and the cell-sorted slot of
+// the first candidate of their chunks (the chunks are those of k_density_brick: 32 candidates from the start of a run)
+// go into the thread's column of a shared table of kTabCap entries; a full table is consumed before the walk goes on.
+// Main loop: the thread walks the table's words as ONE bit stream -- next set bit -> slot -> two 16-byte gathers from
+// global memory (L1 / L2) -- two neighbours per trip on packed binary32, so a lane's trips are half its neighbour count
+// whatever the spread of the bits over the chunks, and no lane waits for another lane's chunk.  A particle with more
+// chunks than mask words walks the grid instead.  (A brick-staged consumer, k_force_brick, with the neighbours'
+// records gathered from shared memory was built and measured: 250 us against 192 us at config 4, 6.6 ms against
+// 2.1 ms at config 5 where its bricks split down to a few cells; DESIGN.md section 10.  It is not kept.)
 constexpr int kMThreads = 128;
 
 __global__ void __launch_bounds__(kMThreads)
@@ -698,14 +554,6 @@ uint32_t brick_blocks(const GridDesc& g) {
 // Staging capacity (particles of a box's neighbourhood).  A brick of config 4 holds 144 cells x 8 = 1152 particles; a
 // box that exceeds the capacity is split, so the choice only moves where the split happens.
 constexpr uint32_t kBrickCap = 2048;   // k_density_brick: 24 KB of x / y / z
-constexpr uint32_t kBrickCapF = 1536;  // k_force_brick: 48 KB of {pos | vel, 1/rho} + 24 KB of word tables: three blocks per SM
-
-static size_t force_smem() { return (size_t)kBrickCapF * 32 + (size_t)kTabCap * kFThreads * 6; }
-
-void brick_init() {
-  cudaFuncSetAttribute(k_force_brick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)force_smem());
-}
-
 void launch_density_brick(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
                           uint32_t* ncount_out, uint32_t* masks, cudaStream_t s, Prof* prof) {
   if (n == 0) return;
@@ -716,23 +564,16 @@ void launch_density_brick(const SphConst& c, const GridBuf& b, uint32_t n, float
   prof->end(s);
 }
 
-void launch_force_brick(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
+void launch_force_masks(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                         uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
-                        uint32_t* touched_out, const uint32_t* masks, bool staged, cudaStream_t s, Prof* prof) {
+                        uint32_t* touched_out, const uint32_t* masks, cudaStream_t s, Prof* prof) {
   if (n == 0) return;
   BoidConst dummy = {};
   const bool has = nb > 0 && bc != nullptr;
-  if (staged) {
-    prof->begin(K_FORCE_BRICK, s);
-    k_force_brick<<<brick_blocks(c.grid), kFThreads, force_smem(), s>>>(
-        c, has ? *bc : dummy, has, pg.posS, pg.velS, pg.start, pg.perm, rhoS, masks, bg.posS, bg.velS, rho_bS, bg.start,
-        pos, vel, accel_out, touched_out, kBrickCapF);
-  } else {
-    prof->begin(K_FORCE_MASKS, s);
-    k_force_masks<<<(n + kMThreads - 1) / kMThreads, kMThreads, 0, s>>>(
-        c, has ? *bc : dummy, has, pg.posS, pg.velS, pg.start, pg.perm, n, rhoS, masks, bg.posS, bg.velS, rho_bS,
-        bg.start, pos, vel, accel_out, touched_out);
-  }
+  prof->begin(K_FORCE_MASKS, s);
+  k_force_masks<<<(n + kMThreads - 1) / kMThreads, kMThreads, 0, s>>>(
+      c, has ? *bc : dummy, has, pg.posS, pg.velS, pg.start, pg.perm, n, rhoS, masks, bg.posS, bg.velS, rho_bS,
+      bg.start, pos, vel, accel_out, touched_out);
   prof->end(s);
 }
 

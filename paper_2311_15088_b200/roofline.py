@@ -30,19 +30,14 @@ def kernel_bytes(n, c, nb, cb, g, t):
         # S7: read bpos 16, write rho_b 4 (the fluid it gathers is already counted)
         "k_boid_density": 20 * nb,
         # S8-S10: read posS 16, velS 16, rho 4, perm 4; write pos' 16, vel' 16
-        "k_force_integrate": 72 * n,
         "k_force_list": 72 * n,     # the stored-neighbour-list variant of the same rows
         "k_density_brick": 20 * n + 8 * c,   # S6 with a brick of cells staged per block (sph_brick.cu)
-        "k_force_brick": 72 * n,
         "k_force_masks": 72 * n,
         # S11-S13: read bpos, bvel 32, rho_b 4, perm 4; write 32
         "k_boid_step": 72 * nb,
         # S14: write phi 4 per corner; read posS 16 per particle and the cell table 8 per cell
         "k_voxel_sdf": 4 * v + 16 * n + 8 * c,
-        "k_voxel_sdf_groups": 4 * v + 16 * n + 8 * c,   # the warp-per-cell-group variant of the same row
-        "k_voxel_sdf_blocks": 4 * v + 16 * n + 8 * c,   # the warp-per-corner-block variant of the same row
         "k_voxel_sdf_tiles": 4 * v + 16 * n + 8 * c,    # the 2x2x2-corners-per-lane tile variant of the same row
-        "k_sdf_axis_tables": 0,                         # helper of S14 (axis partition tables): bytes counted above
         # S15-S17: read phi 4 per corner, write 36 per triangle
         "k_mc_signs": 4 * v,                            # S15 first half: read phi once -> 1 bit per corner
         "k_mc_count": v // 8,                           # S15 second half - S16 on the bit field (1 bit per corner)
@@ -57,7 +52,7 @@ def kernel_bytes(n, c, nb, cb, g, t):
 
 SIM_KERNELS = ("k_hash_count", "k_scan_cells", "k_scatter", "k_reorder", "k_hash_count[boid grid]",
                "k_scan_cells[boid grid]", "k_scatter[boid grid]", "k_reorder[boid grid]", "k_density",
-               "k_boid_density", "k_force_integrate", "k_boid_step")
+               "k_boid_density", "k_force_list", "k_boid_step")
 # The surface pass in SURVEY.md 8(d)'s accounting: phi written once and read once (4 + 4 B per corner), particles and
 # cell table read once, 36 B per triangle.  The fused path reads the sign bits instead of phi (k_mc_signs does not run),
 # but the pass figure keeps the survey's 8 B per corner so that it stays comparable.
@@ -103,9 +98,9 @@ FLOP_PER_PAIR = {
     # three components of (pterm d - 40 mu dv) scaled and accumulated (12)
     "force": 35,
 }
-KERNEL_KIND = {"k_density_brick": "density", "k_force_brick": "force", "k_force_masks": "force",
-               "k_voxel_sdf_tiles": "sdf", "k_voxel_sdf_blocks": "sdf", "k_voxel_sdf_groups": "sdf", "k_voxel_sdf": "sdf",
-               "k_density": "density", "k_force_list": "force", "k_force_integrate": "force"}
+KERNEL_KIND = {"k_density_brick": "density", "k_force_masks": "force",
+               "k_voxel_sdf_tiles": "sdf", "k_voxel_sdf": "sdf",
+               "k_density": "density", "k_force_list": "force"}
 
 
 def sdf_pairs(n, radius, spacing):

@@ -20,7 +20,7 @@ def host_u32(t):
     return t.cpu().numpy().view(np.uint32)
 
 
-FORCE_VARIANT = None  # set by a test fixture: 0 = stored neighbour list, 1 = grid walk, 2 = list from k_density_pairs (sph_set_force_variant)
+FORCE_VARIANT = None  # set by a test fixture: 0 = stored neighbour list, 1 = brick density + neighbour masks (sph_set_force_variant)
 
 
 class Sim:

@@ -17,9 +17,10 @@ from tests.gpuutil import Sim, dev, vec_err
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(autouse=True, params=[0, 1, 2, 3, 4], ids=["nbrlist", "gridwalk", "nbrlist-pairs", "brick", "masks"])
+@pytest.fixture(autouse=True, params=[0, 1], ids=["nbrlist", "masks"])
 def force_variant(request):
-    """Every test runs on both S8 kernels: the stored-neighbour-list pass (default) and the grid walk."""
+    """Every test runs on both S6 / S8 paths: the stored 16-bit neighbour list (default) and the brick density pass with
+    neighbour masks (sph_set_force_variant)."""
     gpuutil.FORCE_VARIANT = request.param
     yield request.param
     gpuutil.FORCE_VARIANT = None
@@ -132,36 +133,6 @@ def test_full_size_step_matches_oracle(idx):
     _compare_step(cfg, out, ref, cfg["pos"])
 
 
-@pytest.mark.parametrize("case", ["config2", "sparse", "ragged"])
-def test_pair_density_is_bitwise_the_per_particle_density(case, force_variant):
-    """k_density_pairs (two targets of a cell per thread, packed binary32) performs every pair's operations in the order
-    of k_density: density, neighbour counts and the state after the step are identical bit for bit.  'sparse' has ~1
-    particle per cell (a warp's 56 slots hold more than 32 pairs: second round); 'ragged' ends inside a warp's slots."""
-    if force_variant != 2:
-        pytest.skip("compares variant 2 with variant 0 once")
-    if case == "config2":
-        cfg = W.config(2)
-        pos0, vel0 = cfg["pos"].copy(), W.uniform_box(cfg["n"], (-0.2,) * 3, (0.2,) * 3, 3, 31)
-    else:
-        cfg = W.config(1)
-        n = 4096 if case == "sparse" else 56 * 37 + 29
-        cfg = dict(cfg, n=n, n_boid=0)
-        pos0 = W.uniform_box(n, (0.0,) * 3, (1.0,) * 3, 5, 32) if case == "sparse" else cfg["pos"][:n].copy()
-        vel0 = W.uniform_box(n, (-0.2,) * 3, (0.2,) * 3, 6, 33)
-    outs = []
-    for v in (0, 2):
-        gpuutil.FORCE_VARIANT = v
-        with Sim(cfg) as sim:
-            outs.append(sim.step(dev(pos0), dev(vel0)))
-    gpuutil.FORCE_VARIANT = 2
-    for k in ("density", "ncount", "accel", "pos", "vel"):
-        assert np.array_equal(outs[0][k], outs[1][k]), k
-    ref = R.step(cfg["sph"], pos0, vel0)
-    assert np.array_equal(outs[1]["ncount"], ref["ncount"])
-    bad, worst = vec_err(outs[1]["density"], ref["density"])
-    assert bad == 0, ("density", bad, worst)
-
-
 @pytest.mark.parametrize("idx,frames", [(2, 100), (3, 100), (4, 100), (5, 20)])
 def test_free_running_frames_as_baseline_states_them(idx, frames, force_variant):
     """BASELINE.json configs[1..4] with the particle, boid and step counts they state (65 536 / 256 / 100, 262 144 / 1 024 /
@@ -170,8 +141,8 @@ def test_free_running_frames_as_baseline_states_them(idx, frames, force_variant)
     for velocities).  Measured on B200 after 100 frames of config 2: max |dpos| 2.7e-7, max |dvel| 8.7e-7, two neighbour
     counts off by one, so a fixed bound of ten single-step floors is asserted at the end as well; the neighbour counts
     (integers decided on r^2 < h^2) may differ only where a pair sits within rounding of h."""
-    if force_variant == 1 or (force_variant == 2 and idx != 2):
-        pytest.skip("the default list variant runs every config, the pair variant config 2; the grid walk has the 10-step test")
+    if force_variant == 1 and idx not in (2, 5):
+        pytest.skip("the default path runs every config, the mask path configs 2 and 5 (the dense one)")
     cfg = W.config(idx)
     rp, rv, rbp, rbv = cfg["pos"], cfg["vel"], cfg["bpos"], cfg["bvel"]
     with Sim(cfg) as sim:

@@ -80,12 +80,12 @@ def test_roofline_bytes_match_survey_totals():
     from paper_2311_15088_b200 import roofline as RF
     n, c = 1 << 20, 1 << 18
     kb = RF.kernel_bytes(n, c, 0, 0, 256, 1_500_000)
-    sph = sum(kb[k] for k in ("k_hash_count", "k_scan_cells", "k_reorder", "k_density", "k_force_integrate"))
+    sph = sum(kb[k] for k in ("k_hash_count", "k_scan_cells", "k_reorder", "k_density", "k_force_list"))
     assert sph == 184 * n + 16 * c  # 184 B + 16 B C/N per particle-step
     mc = RF.pass_bytes(RF.MC_KERNELS, n, c, 0, 0, 256, 1_500_000)
     assert mc == 8 * 256 ** 3 + 16 * n + 8 * c + 36 * 1_500_000
-    rows, dom = RF.summarise({"k_density": (10, 5.0), "k_force_integrate": (10, 15.0)}, n, c, 0, 0, 256, 0, 6557.4)
-    assert dom == "k_force_integrate" and abs(rows[0]["share"] - 0.75) < 1e-12
+    rows, dom = RF.summarise({"k_density": (10, 5.0), "k_force_list": (10, 15.0)}, n, c, 0, 0, 256, 0, 6557.4)
+    assert dom == "k_force_list" and abs(rows[0]["share"] - 0.75) < 1e-12
     assert abs(rows[0]["gbs"] - 72 * n / 1.5e-3 / 1e9) < 1e-6
 
 
