@@ -371,7 +371,7 @@ __device__ __forceinline__ void density_box(const SphConst& c, BrickTab& tb, con
   }
 }
 
-__global__ void __launch_bounds__(kDThreads) k_density_brick(SphConst c, const float4* __restrict__ posS,
+__global__ void __launch_bounds__(kDThreads, 8) k_density_brick(SphConst c, const float4* __restrict__ posS,
                                                              const uint32_t* __restrict__ start,
                                                              const uint32_t* __restrict__ perm,
                                                              float* __restrict__ rhoS, float4* __restrict__ velS,
