@@ -62,43 +62,6 @@ __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, uint32_t lane) {
   return v;
 }
 
-// Bounds of the runs of box b (global slots), their lengths scanned; ends with a barrier.  Cells outside the grid are
-// empty (D:A-BOUND): a run is clipped in x, a row outside in y or z has no particles.
-__device__ __forceinline__ void brick_bounds(BrickTab& tb, const Box& b, const GridDesc& g,
-                                             const uint32_t* __restrict__ start) {
-  const int tid = threadIdx.x, nthreads = blockDim.x;
-  const int ny = b.sy + 2, nrows = ny * (b.sz + 2), nb = b.sx + 3;
-  for (int idx = tid; idx < nrows * nb; idx += nthreads) {
-    const int r = idx / nb, hx = idx - r * nb;
-    const int y = b.y0 - 1 + r % ny, z = b.z0 - 1 + r / ny;
-    uint32_t v = 0;
-    if (y >= 0 && y < g.dim[1] && z >= 0 && z < g.dim[2]) {
-      const int x = min(max(b.x0 - 1 + hx, 0), g.dim[0]);
-      v = __ldg(start + (uint32_t)g.dim[0] * ((uint32_t)y + (uint32_t)g.dim[1] * (uint32_t)z) + (uint32_t)x);
-    }
-    tb.cs[r][hx] = v;
-  }
-  block_sync();
-  if (tid < 32) {
-    const bool row = tid < nrows;
-    const uint32_t a = row ? tb.cs[tid][0] : 0u, e = row ? tb.cs[tid][nb - 1] : 0u;
-    const uint32_t len = e - a;
-    const uint32_t inc = warp_incl_scan(len, (uint32_t)tid);
-    if (row) {
-      tb.g0[tid] = a;
-      tb.off[tid] = inc - len;
-    }
-    if (tid == nrows - 1) tb.off[nrows] = inc;
-    if (tid == 31) tb.T = inc;
-    const int hy = tid % ny, hz = tid / ny;
-    const bool inside = row && hy >= 1 && hy <= b.sy && hz >= 1 && hz <= b.sz;
-    uint32_t nt = inside ? tb.cs[tid][b.sx + 1] - tb.cs[tid][1] : 0u;
-    nt = warp_sum_u32(nt);
-    if (tid == 0) tb.ntarget = nt;
-  }
-  block_sync();
-}
-
 // Copy the runs into shared memory and turn the bounds into staged indices; ends with a barrier.  Positions are staged
 // as three float arrays x[cap], y[cap], z[cap]: two candidates per 8-byte load, and the runs of x-adjacent cells start
 // 32 bytes apart on the rest lattice, so the lanes of a warp hit different banks (with float4 records they start 128
@@ -137,15 +100,18 @@ __device__ __forceinline__ void brick_begin(BrickTab& tb, const GridDesc& g) {
   block_sync();
 }
 
-// One round of the box loop.  Thread 0 alone pops the box and, once the block has computed its bounds, decides what
-// happens to it; the decision travels through shared memory, so every thread acts on the same one.  Boxes without
-// targets are dropped; a box whose neighbourhood exceeds `cap` particles is split (z, then y, then x) unless it is one
-// cell, which is then processed from global memory.
+// One round of the box loop: thread 0 pops a box, the block loads the bounds of its runs (global slots; cells outside the
+// grid are empty, D:A-BOUND: a run is clipped in x, a row outside in y or z has no particles), and warp 0 scans the run
+// lengths, counts the targets, lays out the density pass's units (pairs of targets of one cell) and decides what happens
+// to the box -- the decision is lane 0's and travels through shared memory, so every thread acts on the same one.  A box
+// without targets is dropped; a box whose neighbourhood exceeds `cap` particles is split (z, then y, then x) unless it
+// is one cell, which is then processed from global memory.  Three barriers per round.
 enum { kActDone = 0, kActSkip = 1, kActStaged = 2, kActGlobal = 3 };
 
 __device__ __forceinline__ int brick_round(BrickTab& tb, Box& b, const GridDesc& g, const uint32_t* __restrict__ start,
                                            uint32_t cap) {
-  if (threadIdx.x == 0) {
+  const int tid = threadIdx.x, nthreads = blockDim.x;
+  if (tid == 0) {
     if (tb.sp == 0) {
       tb.action = kActDone;
     } else {
@@ -157,29 +123,68 @@ __device__ __forceinline__ int brick_round(BrickTab& tb, Box& b, const GridDesc&
   block_sync();
   if (tb.action == kActDone) return kActDone;
   b = tb.cur;
-  brick_bounds(tb, b, g, start);
-  if (threadIdx.x == 0) {
-    int act = kActSkip;
-    if (tb.ntarget != 0) {
-      if (tb.T <= cap) {
-        act = kActStaged;
-      } else if (b.sx * b.sy * b.sz == 1) {
-        act = kActGlobal;
-      } else {
-        Box lo = b, hi = b;
-        if (b.sz > 1) {
-          lo.sz = b.sz / 2, hi.sz = b.sz - lo.sz, hi.z0 = b.z0 + lo.sz;
-        } else if (b.sy > 1) {
-          lo.sy = b.sy / 2, hi.sy = b.sy - lo.sy, hi.y0 = b.y0 + lo.sy;
-        } else {
-          lo.sx = b.sx / 2, hi.sx = b.sx - lo.sx, hi.x0 = b.x0 + lo.sx;
-        }
-        tb.stack[tb.sp] = hi;
-        tb.stack[tb.sp + 1] = lo;
-        tb.sp += 2;
-      }
+  const int ny = b.sy + 2, nrows = ny * (b.sz + 2), nb = b.sx + 3;
+  for (int idx = tid; idx < nrows * nb; idx += nthreads) {
+    const int r = idx / nb, hx = idx - r * nb;
+    const int y = b.y0 - 1 + r % ny, z = b.z0 - 1 + r / ny;
+    uint32_t v = 0;
+    if (y >= 0 && y < g.dim[1] && z >= 0 && z < g.dim[2]) {
+      const int x = min(max(b.x0 - 1 + hx, 0), g.dim[0]);
+      v = __ldg(start + (uint32_t)g.dim[0] * ((uint32_t)y + (uint32_t)g.dim[1] * (uint32_t)z) + (uint32_t)x);
     }
-    tb.action = act;
+    tb.cs[r][hx] = v;
+  }
+  block_sync();
+  if (tid < 32) {
+    const bool row = tid < nrows;
+    const uint32_t a = row ? tb.cs[tid][0] : 0u, e = row ? tb.cs[tid][nb - 1] : 0u;
+    const uint32_t len = e - a;
+    const uint32_t inc = warp_incl_scan(len, (uint32_t)tid);
+    if (row) {
+      tb.g0[tid] = a;
+      tb.off[tid] = inc - len;
+    }
+    if (tid == nrows - 1) tb.off[nrows] = inc;
+    const uint32_t T = __shfl_sync(kFull, inc, 31);
+    const int hy = tid % ny, hz = tid / ny;
+    const bool inside = row && hy >= 1 && hy <= b.sy && hz >= 1 && hz <= b.sz;
+    const uint32_t nt = warp_sum_u32(inside ? tb.cs[tid][b.sx + 1] - tb.cs[tid][1] : 0u);
+    // units of the density pass before each cell of the box (cell = lane, x fastest); differences of bounds, so the
+    // raw global slots serve
+    uint32_t u = 0;
+    if (tid < b.sx * b.sy * b.sz) {
+      const int lx = tid % b.sx, ly = (tid / b.sx) % b.sy, lz = tid / (b.sx * b.sy);
+      const int r = (ly + 1) + ny * (lz + 1);
+      u = (tb.cs[r][lx + 2] - tb.cs[r][lx + 1] + 1u) >> 1;
+    }
+    const uint32_t uinc = warp_incl_scan(u, (uint32_t)tid);
+    tb.pre[tid] = uinc - u;
+    if (tid == 31) tb.pre[32] = uinc;
+    if (tid == 0) {
+      tb.T = T;
+      tb.ntarget = nt;
+      int act = kActSkip;
+      if (nt != 0) {
+        if (T <= cap) {
+          act = kActStaged;
+        } else if (b.sx * b.sy * b.sz == 1) {
+          act = kActGlobal;
+        } else {
+          Box lo = b, hi = b;
+          if (b.sz > 1) {
+            lo.sz = b.sz / 2, hi.sz = b.sz - lo.sz, hi.z0 = b.z0 + lo.sz;
+          } else if (b.sy > 1) {
+            lo.sy = b.sy / 2, hi.sy = b.sy - lo.sy, hi.y0 = b.y0 + lo.sy;
+          } else {
+            lo.sx = b.sx / 2, hi.sx = b.sx - lo.sx, hi.x0 = b.x0 + lo.sx;
+          }
+          tb.stack[tb.sp] = hi;
+          tb.stack[tb.sp + 1] = lo;
+          tb.sp += 2;
+        }
+      }
+      tb.action = act;
+    }
   }
   block_sync();
   return tb.action;
@@ -227,21 +232,9 @@ __device__ __forceinline__ void density_box(const SphConst& c, BrickTab& tb, con
                                             float* __restrict__ density_out, uint32_t* __restrict__ ncount_out,
                                             uint32_t* __restrict__ masks) {
   const int tid = threadIdx.x;
-  const int ny = b.sy + 2, ncell = b.sx * b.sy * b.sz;
+  const int ny = b.sy + 2;
   const float* sy = sx + cap;
   const float* sz = sx + 2u * cap;
-  if (tid < 32) {  // units (pairs of targets of one cell) before each cell
-    uint32_t u = 0;
-    if (tid < ncell) {
-      const int lx = tid % b.sx, ly = (tid / b.sx) % b.sy, lz = tid / (b.sx * b.sy);
-      const int r = (ly + 1) + ny * (lz + 1);
-      u = (tb.cs[r][lx + 2] - tb.cs[r][lx + 1] + 1u) >> 1;
-    }
-    const uint32_t inc = warp_incl_scan(u, (uint32_t)tid);
-    tb.pre[tid] = inc - u;
-    if (tid == 31) tb.pre[32] = inc;
-  }
-  block_sync();
   const uint32_t U = tb.pre[32];
   const f32x2 neg_h2 = pack2(-c.h2, -c.h2);
 #pragma unroll 1
