@@ -85,6 +85,12 @@ uint32_t sph_grid_dims(const sph_ctx* ctx, uint32_t dims_out[3] /* host */);
 int sph_build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, void* stream,
                    uint32_t* cell_of_particle, uint32_t* perm, uint32_t* cell_start);
 
+/* Bounding box of the particles of the last sph_build_grid (the grid build computes it on the device; the surface pass
+ * uses it to skip corner tiles beyond R of every particle).  lo_hi_host = 6 host floats: min x, y, z, max x, y, z, exact
+ * (binary32 min / max of the coordinates).  Synchronises `stream`.  SPH_E_STALE_GRID without a current grid or with no
+ * particles.  Lets a caller lay the voxel grid over the fluid's bounding box at extraction time (BASELINE config 4). */
+int sph_particle_aabb(sph_ctx* ctx, void* stream, float* lo_hi_host);
+
 /* S6-S10: one SPH step, in place on pos / vel.
  *   density rho_i = sum_j m W_poly6 (self included), neighbour count;
  *   f_i = sum_j Listing-3 pair term; boids push the fluid (D:C-COUPLE); a_i = f_i/rho_i + g (D:A-RHO);

@@ -427,6 +427,21 @@ int sph_build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, v
   return SPH_OK;
 }
 
+int sph_particle_aabb(sph_ctx* ctx, void* stream, float* lo_hi_host) {
+  if (!ctx || !lo_hi_host) return SPH_E_INVALID;
+  if (!ctx->grid_fresh || ctx->grid_n == 0) return fail(ctx, SPH_E_STALE_GRID, "no current grid (or no particles)");
+  cudaStream_t s = (cudaStream_t)stream;
+  CK(cudaSetDevice(ctx->device));
+  uint32_t e[6];
+  CK(cudaMemcpyAsync(e, ctx->pg.aabb_now, sizeof(e), cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
+  for (int a = 0; a < 6; ++a) {  // inverse of encode_ordered (common.cuh)
+    const uint32_t b = (e[a] & 0x80000000u) ? (e[a] & 0x7fffffffu) : ~e[a];
+    memcpy(lo_hi_host + a, &b, 4);
+  }
+  return SPH_OK;
+}
+
 int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, const void* bvel, uint32_t n_boid,
              const boid_params* bp, void* stream, float* density, void* accel, uint32_t* ncount, uint32_t* touched) {
   if (!ctx) return SPH_E_INVALID;

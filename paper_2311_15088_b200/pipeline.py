@@ -19,7 +19,11 @@ from . import workloads as W
 
 
 class Frame:
-    def __init__(self, cfg, device=0, tri_capacity=None, with_mc=True):
+    def __init__(self, cfg, device=0, tri_capacity=None, with_mc=True, track_aabb=False):
+        """track_aabb: lay the voxel grid over the fluid's bounding box AT EXTRACTION TIME (BASELINE config 4 / 5: 'MC
+        256^3 over the fluid bounding box'): after every grid build the box is read back from the device
+        (sph_particle_aabb, one small synchronising copy per frame) and origin / spacing follow it.  Off by default:
+        the grid then stays where the initial state put it, and a frame enqueues without any host synchronisation."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2311_15088_b200 needs a CUDA device (there is no CPU fallback)")
@@ -29,6 +33,7 @@ class Frame:
         torch.cuda.set_device(self.device)
         self.n, self.nb = cfg["n"], cfg["n_boid"]
         self.with_mc = with_mc
+        self.track_aabb = bool(track_aabb) and with_mc and cfg.get("idx") in (4, 5)
         self.mc = W.mc_params(cfg) if with_mc else None
         self.G = self.mc["n_point_per_axis"] if with_mc else 0
         self.ctx = B.sph_create(cfg["sph"], max(self.n, 1), max(self.nb, 1), self.G, device=device)
@@ -52,6 +57,10 @@ class Frame:
         if self.nb:
             B.boid_step(self.ctx, self.cfg["boid"], self.bpos, self.bvel)
         B.sph_build_grid(self.ctx, self.pos, self.vel)
+        if self.track_aabb:
+            lo, hi = B.sph_particle_aabb(self.ctx)
+            extent = max(np.float32(hi[a]) - np.float32(lo[a]) for a in range(3))
+            self.mc = dict(self.mc, origin=tuple(float(x) for x in lo), spacing=float(np.float32(extent / (self.G - 1))))
 
     def surface(self, sync=False):
         """S14-S17 on the current grid.  Returns the triangle count when sync."""

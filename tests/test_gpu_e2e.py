@@ -153,3 +153,28 @@ def test_simulate_host_three_steps_is_bitwise_the_device_path(pinned):
         B.sph_simulate_host(sim.ctx, again[0], again[1], again[2], again[3], cfg["boid"], 0, None, None)
         for g, k in zip(again, ("pos", "vel", "bpos", "bvel")):
             assert np.array_equal(g.numpy(), np.ascontiguousarray(cfg[k]))
+
+
+def test_particle_aabb_is_exact_and_frame_can_follow_it():
+    """sph_particle_aabb returns the exact binary32 bounding box of the particles the grid was built on, and
+    Frame(track_aabb=True) lays config 4's voxel grid over the fluid box at extraction time (workloads.mc_params on the
+    current positions), not over the initial one."""
+    import numpy as np
+    import torch
+    from paper_2311_15088_b200 import binding as B
+    from paper_2311_15088_b200 import workloads as W
+    from paper_2311_15088_b200.pipeline import Frame
+    cfg = W.config(4, scale=4)
+    with Frame(cfg, track_aabb=True) as fr:
+        with pytest.raises(B.SphError) as e:
+            B.sph_particle_aabb(fr.ctx)
+        assert e.value.code == B.SPH_E_STALE_GRID
+        for _ in range(30):
+            fr.frame()
+        torch.cuda.synchronize()
+        p = fr.pos.cpu().numpy()
+        lo, hi = B.sph_particle_aabb(fr.ctx)
+        assert np.array_equal(np.float32(lo), p[:, :3].min(axis=0)) and np.array_equal(np.float32(hi), p[:, :3].max(axis=0))
+        want = W.mc_params(cfg, p)
+        assert fr.mc["origin"] == want["origin"] and fr.mc["spacing"] == want["spacing"]
+        assert fr.mc["origin"] != W.mc_params(cfg)["origin"] or fr.mc["spacing"] != W.mc_params(cfg)["spacing"]
