@@ -85,6 +85,10 @@ uint32_t sph_grid_dims(const sph_ctx* ctx, uint32_t dims_out[3] /* host */);
 int sph_build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, void* stream,
                    uint32_t* cell_of_particle, uint32_t* perm, uint32_t* cell_start);
 
+/* Forget the current grid: the next sph_step rebuilds it, the next mc_* call returns SPH_E_STALE_GRID until
+ * sph_build_grid is called.  For callers that rewrite pos in place between sph_build_grid and sph_step / mc_*. */
+int sph_invalidate_grid(sph_ctx* ctx);
+
 /* Bounding box of the particles of the last sph_build_grid (the grid build computes it on the device; the surface pass
  * uses it to skip corner tiles beyond R of every particle).  lo_hi_host = 6 host floats: min x, y, z, max x, y, z, exact
  * (binary32 min / max of the coordinates).  Synchronises `stream`.  SPH_E_STALE_GRID without a current grid or with no
@@ -95,7 +99,10 @@ int sph_particle_aabb(sph_ctx* ctx, void* stream, float* lo_hi_host);
  *   density rho_i = sum_j m W_poly6 (self included), neighbour count;
  *   f_i = sum_j Listing-3 pair term; boids push the fluid (D:C-COUPLE); a_i = f_i/rho_i + g (D:A-RHO);
  *   v += a dt, x += v dt (Euler-Cromer), damped wall clamp (D:A-WALL).
- * Builds the grid itself unless the last sph_build_grid was on this (pos, vel, n).
+ * Builds the grid itself unless the last sph_build_grid was on this (pos, vel, n) -- "this" means the same POINTERS and
+ * count, and the library trusts that the arrays were not rewritten in between: a caller that modifies pos in place after
+ * sph_build_grid (or whose allocator hands a new array the old address) must call sph_invalidate_grid first, otherwise
+ * the step runs on the stale sort.  The mc_* calls trust the same flag.
  * bpos / bvel [n_boid] are the step-start boids (not modified); bp may be NULL iff n_boid == 0.
  * Optional outputs in caller order (NULL to skip): density[n], accel[n] (float4, total a_i),
  * ncount[n], touched[n] (number of boids inside the push radius). */

@@ -87,6 +87,7 @@ def lib():
         L.sph_hashgrid_neighbor_count.argtypes = [_vp, _vp, _u32, _u32, _vp, _vp, _vp]
         L.sph_set_force_variant.argtypes = [_vp, C.c_int]
         L.sph_particle_aabb.argtypes = [_vp, _vp, _vp]
+        L.sph_invalidate_grid.argtypes = [_vp]
         L.mc_polygonise.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.mc_extract.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32, _vp]
         L.mc_extract_async.argtypes = [_vp, _vp, _vp, _vp, _vp, _u32]
@@ -108,7 +109,7 @@ def lib():
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
-           "sph_particle_aabb", "mc_voxel_sdf", "mc_set_sdf_variant", "mc_set_cube_range", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_pack_range", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "mc_mesh_components", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
+           "sph_particle_aabb", "sph_invalidate_grid", "mc_voxel_sdf", "mc_set_sdf_variant", "mc_set_cube_range", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_pack_range", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "mc_mesh_components", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
            "sph_profile_read", "sph_kernel_name"]
 
 
@@ -253,6 +254,10 @@ def sph_hashgrid_neighbor_count(ctx, pos, max_per_cell, ncount, stream=None, syn
     _check(ctx, lib().sph_hashgrid_neighbor_count(ctx, _ptr(pos), pos.shape[0], int(max_per_cell), _stream(stream),
                                                   _ptr(ncount), C.byref(dropped) if sync else None))
     return int(dropped.value) if sync else None
+
+
+def sph_invalidate_grid(ctx):
+    return _check(ctx, lib().sph_invalidate_grid(ctx))
 
 
 def sph_particle_aabb(ctx, stream=None):

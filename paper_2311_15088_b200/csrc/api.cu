@@ -427,6 +427,13 @@ int sph_build_grid(sph_ctx* ctx, const void* pos, const void* vel, uint32_t n, v
   return SPH_OK;
 }
 
+int sph_invalidate_grid(sph_ctx* ctx) {
+  if (!ctx) return SPH_E_INVALID;
+  ctx->grid_fresh = false;
+  ctx->grid_pos = ctx->grid_vel = nullptr;
+  return SPH_OK;
+}
+
 int sph_particle_aabb(sph_ctx* ctx, void* stream, float* lo_hi_host) {
   if (!ctx || !lo_hi_host) return SPH_E_INVALID;
   if (!ctx->grid_fresh || ctx->grid_n == 0) return fail(ctx, SPH_E_STALE_GRID, "no current grid (or no particles)");

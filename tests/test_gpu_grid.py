@@ -85,3 +85,30 @@ def test_neighbor_counts_sorted_and_hashgrid_match_oracle(idx, scale):
         cnt2 = torch.zeros_like(cnt)
         dropped = B.sph_hashgrid_neighbor_count(sim.ctx, pos, 4, cnt2)
         assert dropped > 0 and bool((cnt2 <= cnt).all()) and bool((cnt2 < cnt).any())
+
+
+def test_invalidate_grid_after_rewriting_positions_in_place():
+    """sph_step reuses a grid by pointer identity (include/sphboid.h): a caller that rewrites pos in place after
+    sph_build_grid must call sph_invalidate_grid, after which the step sorts the new positions; mc_* then refuses the
+    stale grid."""
+    import torch
+    from oracle import refbind as R
+    from paper_2311_15088_b200 import binding as B
+    from tests.gpuutil import vec_err
+    cfg = W.config(1)
+    other = W.uniform_box(cfg["n"], (0.1,) * 3, (0.6,) * 3, 3, 77)
+    ref = R.step(cfg["sph"], other, cfg["vel"])
+    with Sim(cfg, G=16) as sim:
+        pos, vel = dev(cfg["pos"]), dev(cfg["vel"])
+        B.sph_build_grid(sim.ctx, pos, vel)
+        pos.copy_(dev(other))            # same pointer, new contents
+        B.sph_invalidate_grid(sim.ctx)
+        mp = dict(origin=(0.0, 0.0, 0.0), spacing=1.0 / 15, n_point_per_axis=16, radius=cfg["sph"]["h"],
+                  particle_radius=0.5 * cfg["sph"]["h"], iso=0.0)
+        with pytest.raises(B.SphError) as e:
+            B.mc_voxel_sdf(sim.ctx, mp, torch.zeros(16 ** 3, device="cuda"))
+        assert e.value.code == B.SPH_E_STALE_GRID
+        out = sim.step(pos, vel)
+    assert np.array_equal(out["ncount"], ref["ncount"])
+    bad, worst = vec_err(out["pos"][:, :3], ref["pos"][:, :3])
+    assert bad == 0, (bad, worst)
