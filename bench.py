@@ -230,8 +230,10 @@ def run_slab(args):
     launches0 = B.sph_launch_count(be.ctx)
     ev[0].record()
     n_tris = 0
-    for _ in range(K):
+    for k in range(K):
         n_tris = sim.step(tris)
+        if args.recut_every and (k + 1) % args.recut_every == 0 and ranks.world > 1:
+            sim.recut()
     ev[1].record()
     torch.cuda.synchronize()
     ranks.barrier()
@@ -270,6 +272,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--force-variant", type=int, default=0, help="A/B: 0 = stored neighbour list (default), 1 = brick density pass + neighbour masks")
     ap.add_argument("--sdf-variant", type=int, default=0, help="A/B: 0 = cost model (default), 1 = per-corner walk, 2 = corner tiles")
+    ap.add_argument("--recut-every", type=int, default=0, help="slab decomposition: re-cut the faces by particle count every k frames (0 = never)")
     ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (default) or the fluid cut into slabs with halo exchange (N2, SPH step only)")
     args = ap.parse_args()

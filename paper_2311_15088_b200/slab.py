@@ -67,15 +67,24 @@ class SlabLayout:
         if pos is None:
             cuts = [self.cells_per_rank * r for r in range(1, self.world)]
         else:
-            x = np.asarray(pos)[:, self.axis].astype(np.float32)
-            col = np.clip(np.floor((x - np.float32(self.origin)) / np.float32(self.h)).astype(np.int64), 0, self.dim - 1)
+            col = self.column_of(np.asarray(pos)[:, self.axis])
             cuts = self.balanced_cuts(np.bincount(col, minlength=self.dim), self.world, min_cells)
+        self.min_cells = min_cells
+        self.set_cuts(cuts)
+
+    def set_cuts(self, cuts):
+        """Move the faces to these cell indices (a re-cut during a run: SlabSim.recut / run_recut)."""
         widths = np.diff([0] + list(cuts) + [self.dim])
-        if self.world > 1 and (len(cuts) != self.world - 1 or (widths < min_cells).any()):
-            raise ValueError("slabs must be at least one halo wide (ghosts come from the two neighbours only)")
+        if self.world > 1 and (len(cuts) != self.world - 1 or (widths < self.min_cells).any()):
+            raise ValueError("slabs must be at least one halo wide")
         self.cuts = [int(c) for c in cuts]
         # faces in binary32, the precision positions are compared in
         self.faces = [float(np.float32(self.origin + np.float32(c) * np.float32(self.h))) for c in self.cuts]
+
+    def column_of(self, x):
+        """Cell column along the slab axis of coordinate(s) x (numpy), clamped like the grid's cells."""
+        x = np.asarray(x, np.float32)
+        return np.clip(np.floor((x - np.float32(self.origin)) / np.float32(self.h)).astype(np.int64), 0, self.dim - 1)
 
     @staticmethod
     def balanced_cuts(hist, world, min_cells):
@@ -142,6 +151,19 @@ class LoopbackExchange:
     def collect(self, rank, tag):
         return self.box.pop((rank, tag, "from_left"), None), self.box.pop((rank, tag, "from_right"), None)
 
+    def post_reduce(self, rank, tag, arr):
+        """Sum of int64 arrays over the ranks (the re-cut's column histogram, its 'anybody still moving' count)."""
+        self.box.setdefault(("sum", tag), []).append(np.asarray(arr, np.int64))
+
+    def collect_reduce(self, rank, tag):
+        parts = self.box[("sum", tag)]
+        assert len(parts) >= self.world, "every rank posts before anybody collects"
+        total = np.sum(parts[:self.world], axis=0)
+        parts.append(None)  # one marker per collector; the entry goes when everybody has collected
+        if len(parts) == 2 * self.world:
+            del self.box[("sum", tag)]
+        return total
+
 
 class DistExchange:
     """torch.distributed neighbour exchange (NCCL on GPUs, gloo on CPU tensors).  Count and payload travel in ONE
@@ -195,6 +217,15 @@ class DistExchange:
             out.append((self.recv[side][1:1 + k, 0:4], self.recv[side][1:1 + k, 4:8]) if k else None)
         return out[0], out[1]
 
+    def post_reduce(self, rank, tag, arr):
+        self.pending[("sum", tag)] = np.asarray(arr, np.int64)
+
+    def collect_reduce(self, rank, tag):
+        import torch
+        t = torch.from_numpy(self.pending.pop(("sum", tag)).copy()).to(self.device)
+        self.dist.all_reduce(t)
+        return t.cpu().numpy()
+
 
 class GpuBackend:
     """Selection and stepping through libsphboid on one GPU (device memory from torch)."""
@@ -218,6 +249,15 @@ class GpuBackend:
             return self.empty(), self.empty()
         k = self.B.sph_pack_range(self.ctx, pos, vel, n, axis, lo, hi, self.scratch[0], self.scratch[1])
         return self.scratch[0][:k].clone(), self.scratch[1][:k].clone()
+
+    def column_hist(self, pos, n, axis, origin, h, dim):
+        """Particles per cell column along `axis` (decomposition bookkeeping, not part of the frame: torch on the device,
+        one small copy to the host)."""
+        t = self.torch
+        if n == 0:
+            return np.zeros(dim, np.int64)
+        col = t.clamp(t.floor((pos[:n, axis] - np.float32(origin)) / np.float32(h)).to(t.int64), 0, dim - 1)
+        return t.bincount(col, minlength=dim).cpu().numpy()
 
     def step(self, pos, vel, bpos=None, bvel=None, boid=None):
         if bpos is None or bpos.shape[0] == 0:
@@ -347,6 +387,53 @@ class SlabSim:
             self.nb_owned = self.bpos.shape[0]
         self.step_no += 1
 
+    # -- re-cut: move the faces to where the particles are now --------------------------------------------------------
+    def post_recut(self):
+        lay = self.layout
+        self._recut_tag = ("recut", self.step_no)
+        self.exchange.post_reduce(self.rank, self._recut_tag,
+                                  self.backend.column_hist(self.pos, self.n_owned, lay.axis, lay.origin, lay.h, lay.dim))
+
+    def apply_recut(self):
+        """New faces from the global column histogram (the same on every rank); returns the new cuts.  The particles and
+        boids that now lie outside the rank's slab are moved by migration rounds (migrate_round) until none is left:
+        a face that moved further than one slab needs more than one."""
+        lay = self.layout
+        hist = self.exchange.collect_reduce(self.rank, self._recut_tag)
+        lay.set_cuts(SlabLayout.balanced_cuts(hist, lay.world, lay.min_cells))
+        self.lo, self.hi = lay.bounds(self.rank)
+        self._round = 0
+        return lay.cuts
+
+    def migrate_round_post(self):
+        self.post_migration()
+
+    def migrate_round_finish(self):
+        """Finishes one migration round and posts how many of this rank's particles / boids are still foreign."""
+        self.finish_migration()
+        self.step_no -= 1  # finish_migration counts a frame; a re-cut round is not one
+        self._round += 1
+        ax, be, inf = self.layout.axis, self.backend, math.inf
+        foreign = self.n_owned - be.pack(self.pos, self.vel, self.n_owned, ax, self.lo, self.hi)[0].shape[0]
+        if self.boid is not None:
+            foreign += self.nb_owned - be.pack(self.bpos, self.bvel, self.nb_owned, ax, self.lo, self.hi)[0].shape[0]
+        self._round_tag = ("recut-left", self.step_no, self._round)
+        self.exchange.post_reduce(self.rank, self._round_tag, [foreign])
+
+    def migrate_round_left(self):
+        return int(self.exchange.collect_reduce(self.rank, self._round_tag)[0])
+
+    def recut(self):
+        """The whole re-cut on one rank (DistExchange: every rank calls it at the same frame)."""
+        self.post_recut()
+        cuts = self.apply_recut()
+        for _ in range(self.layout.world):
+            self.migrate_round_post()
+            self.migrate_round_finish()
+            if self.migrate_round_left() == 0:
+                break
+        return cuts
+
     def step(self, tris=None):
         """One decomposed frame (with DistExchange every rank calls this; with LoopbackExchange drive the phases).
         With tris: the surface of the frame-start state for this rank's cubes first; returns its triangle count."""
@@ -383,3 +470,18 @@ def run_loopback(sims, steps, tris=None):
         for s in sims:
             s.finish_migration()
     return counts
+
+
+def run_recut(sims):
+    """Single-process emulation of SlabSim.recut: all ranks post, then all ranks collect, phase by phase."""
+    for s in sims:
+        s.post_recut()
+    cuts = [s.apply_recut() for s in sims][0]
+    for _ in range(len(sims)):
+        for s in sims:
+            s.migrate_round_post()
+        for s in sims:
+            s.migrate_round_finish()
+        if [s.migrate_round_left() for s in sims][0] == 0:
+            break
+    return cuts

@@ -25,6 +25,11 @@ class OracleBackend:
         sel = torch.from_numpy((x >= np.float32(lo)) & (x < np.float32(hi)))
         return pos[:n][sel].clone(), vel[:n][sel].clone()
 
+    def column_hist(self, pos, n, axis, origin, h, dim):
+        x = pos[:n, axis].numpy()
+        col = np.clip(np.floor((x - np.float32(origin)) / np.float32(h)).astype(np.int64), 0, dim - 1)
+        return np.bincount(col, minlength=dim)
+
     def step(self, pos, vel, bpos=None, bvel=None, boid=None):
         if bpos is None or bpos.shape[0] == 0:
             out = R.step(self.sph, pos.numpy(), vel.numpy())

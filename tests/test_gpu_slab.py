@@ -206,3 +206,48 @@ def test_balanced_slabs_config4_over_8_emulated_ranks():
     assert bad <= n // 10000, ("pos", bad, worst)
     bad, worst = vec_err(gv[:, :3], ref_v[:, :3], rel=1e-5 * steps, abs_=2e-5 * steps)
     assert bad <= n // 10000, ("vel", bad, worst)
+
+
+def test_recut_on_the_gpu_backend_balances_and_keeps_parity():
+    """N2 re-cut with the library as the stepper: config 2 over 4 emulated ranks from UNIFORM slabs (the fluid fills half
+    of the box: two ranks own nothing), one frame, a re-cut from the global column histogram (multi-hop migration), two
+    more frames; owned counts balance and the result matches the undecomposed GPU run."""
+    cfg = W.config(2)
+    world, n = 4, cfg["n"]
+    pos = cfg["pos"].copy()
+    pos[:, 3] = np.arange(n, dtype=np.float32)
+    lay = S.SlabLayout(cfg["sph"], world, boid=cfg["boid"])
+    ex = S.LoopbackExchange(world)
+    backends = [S.GpuBackend(cfg["sph"], n, boid_capacity=cfg["n_boid"]) for _ in range(world)]
+    try:
+        parts, bparts = S.split_initial(lay, pos, cfg["vel"]), S.split_initial(lay, cfg["bpos"], cfg["bvel"])
+        sims = [S.SlabSim(lay, r, backends[r], ex, backends[r].to_device(parts[r][0]), backends[r].to_device(parts[r][1]),
+                          backends[r].to_device(bparts[r][0]), backends[r].to_device(bparts[r][1]), cfg["boid"])
+                for r in range(world)]
+        before = np.array([s.n_owned for s in sims])
+        assert before.max() / before.mean() > 1.9
+        S.run_loopback(sims, 1)
+        S.run_recut(sims)
+        after = np.array([s.n_owned for s in sims])
+        print("owned before", before.tolist(), "after", after.tolist(), "cuts", lay.cuts)
+        assert after.sum() == n and after.max() / after.mean() <= 1.10
+        assert sum(s.nb_owned for s in sims) == cfg["n_boid"]
+        S.run_loopback(sims, 2)
+        got = np.concatenate([np.concatenate([x.pos.cpu().numpy(), x.vel.cpu().numpy()], 1) for x in sims], 0)
+    finally:
+        for b in backends:
+            b.close()
+    with Sim(cfg) as one:
+        dp, dv, dbp, dbv = dev(pos), dev(cfg["vel"]), dev(cfg["bpos"]), dev(cfg["bvel"])
+        for _ in range(3):
+            B.sph_step(one.ctx, dp, dv, dbp, dbv, cfg["boid"])
+            B.boid_step(one.ctx, cfg["boid"], dbp, dbv)
+        ref_p, ref_v = dp.cpu().numpy(), dv.cpu().numpy()
+    ids = got[:, 3].astype(np.int64)
+    assert np.array_equal(np.sort(ids), np.arange(n))
+    gp, gv = np.zeros_like(ref_p), np.zeros_like(ref_v)
+    gp[ids], gv[ids] = got[:, :4], got[:, 4:]
+    bad, worst = vec_err(gp[:, :3], ref_p[:, :3], rel=3e-5, abs_=6e-6)
+    assert bad <= n // 10000, ("pos", bad, worst)
+    bad, worst = vec_err(gv[:, :3], ref_v[:, :3], rel=3e-5, abs_=6e-5)
+    assert bad <= n // 10000, ("vel", bad, worst)

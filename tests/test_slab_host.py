@@ -258,3 +258,40 @@ def test_faces_cut_by_particle_count_balance_config4_over_8_ranks():
     # a histogram with everything in one column cannot be balanced: the cuts fall back to the narrowest legal slabs
     cuts = S.SlabLayout.balanced_cuts(np.array([0, 0, 1000, 0, 0, 0, 0, 0, 0, 0, 0, 0]), 3, 3)
     assert cuts == [3, 6] or (np.diff([0] + cuts + [12]) >= 3).all()
+
+
+def test_recut_moves_the_faces_and_the_particles_two_hops_if_needed():
+    """N2 re-cut (SlabSim.recut / run_recut): three emulated ranks start from uniform cell slabs of config 1 (the fluid
+    fills half of the box: ranks own 3/4, 1/4 and nothing), the faces are re-cut from the global column histogram, the
+    particles move to their new owners -- some from rank 0 to rank 2, two hops -- and the decomposed frames that follow
+    still match the undecomposed oracle."""
+    from oracle import refbind as R
+    from tests.slabutil import OracleBackend, gather_by_id, tagged_state
+    cfg = W.config(1)
+    pos, vel = tagged_state(cfg, speed=2.0)
+    world, n = 3, cfg["n"]
+    lay = S.SlabLayout(cfg["sph"], world)
+    assert lay.cuts == [6, 12]
+    ex = S.LoopbackExchange(world)
+    be = OracleBackend(cfg["sph"])
+    sims = [S.SlabSim(lay, r, be, ex, be.to_device(p), be.to_device(v)) for r, (p, v) in enumerate(S.split_initial(lay, pos, vel))]
+    assert [s.n_owned for s in sims] == [3 * n // 4, n // 4, 0]
+    S.run_loopback(sims, 1)
+    ref = R.step(cfg["sph"], pos, vel)
+    cuts = S.run_recut(sims)
+    assert cuts != [6, 12] and cuts == lay.cuts
+    owned = np.array([s.n_owned for s in sims])
+    assert owned.sum() == n and owned.max() / owned.mean() < 1.35 and owned.min() > 0
+    for s in sims:
+        x = s.pos[:, lay.axis].numpy()
+        lo, hi = lay.bounds(s.rank)
+        assert ((x >= np.float32(lo)) & (x < np.float32(hi))).all()
+    gp, gv = gather_by_id([(s.pos.numpy(), s.vel.numpy()) for s in sims], n)
+    assert np.array_equal(gp, ref["pos"]) or np.abs(gp - ref["pos"]).max() <= 1e-6   # the re-cut moves owners, not particles
+    rp, rv = ref["pos"], ref["vel"]
+    for _ in range(2):
+        S.run_loopback(sims, 1)
+        o = R.step(cfg["sph"], rp, rv)
+        rp, rv = o["pos"], o["vel"]
+    gp, gv = gather_by_id([(s.pos.numpy(), s.vel.numpy()) for s in sims], n)
+    assert np.abs(gp[:, :3] - rp[:, :3]).max() <= 1e-6 and np.abs(gv[:, :3] - rv[:, :3]).max() <= 1e-5
