@@ -99,6 +99,19 @@ class ClockSampler:
         return out
 
 
+def workload_config(cfg, world):
+    """The `config` object of the JSON line: the workload only, identical for the GPU arm and the --impl reference arm
+    (run-specific facts -- frame loop, grid cells, triangle count -- go under `run`)."""
+    n, nb, G = cfg["n"], cfg["n_boid"], cfg["G"]
+    state_bytes = 32 * n * 2 + 16 * n + 4 * G ** 3
+    return {"workload": cfg["name"], "particles": n, "boids": nb, "mc_points_per_axis": G,
+            "parallelism": "replicas x%d" % world,
+            "l2": ("no explicit flush: the frame's working set (%.0f MB of state, sorted copies and phi) exceeds the %.0f MB "
+                   "L2 and the state changes every step" if state_bytes > L2_BYTES else
+                   "no explicit flush, and this workload's working set (%.0f MB) FITS the %.0f MB L2: an L2-resident "
+                   "figure (the headline workload, config4, exceeds it)") % (state_bytes / 1e6, L2_BYTES / 1e6)}
+
+
 def oracle_frame(R, W, cfg, mp, state):
     """One frame on the CPU oracle (same order as Frame.frame).  state = [pos, vel, bpos, bvel]; returns n_tris."""
     pos, vel, bpos, bvel = state
@@ -180,8 +193,8 @@ def run_reference(args, cfg_idx):
         "impl": "reference", "metric": METRIC, "value": value, "unit": "particle-updates/s", "n_gpus": args.gpus,
         "steps": k, "warmup": done_w, "ms_per_step": 1e3 * t / k, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": cfg["name"], "particles": n, "boids": cfg["n_boid"], "mc_points_per_axis": cfg["G"],
-                   "note": "CPU oracle (oracle/, plain C++ with OpenMP over the outer index), one frame per step"},
+        "config": workload_config(cfg, args.gpus),
+        "run": {"note": "CPU oracle (oracle/, plain C++ with OpenMP over the outer index), one frame per step"},
         "cpu_baseline": {"value": value, "unit": "particle-updates/s", "cores": R.num_threads(), "kind": "oracle",
                          "sample": "%d whole frames of %s (steps requested %d, time-capped)" % (k, cfg["name"],
                                                                                               args.steps)},
@@ -540,21 +553,18 @@ def main():
                                                          "time ratio measured on config2)"}}
 
     if ranks.rank == 0:
-        state_bytes = 32 * n * 2 + 16 * n + 4 * G ** 3 + 36 * n_tris + 8 * C
         line = {
             "metric": METRIC, "value": value, "unit": "particle-updates/s", "n_gpus": world, "steps": K,
             "warmup": args.warmup, "ms_per_step": 1e3 * t_max / K, "ms_per_step_pipelined": 1e3 * t_pipe_max / K,
             "ms_per_step_serial": 1e3 * t_serial_max / K, "ms_per_step_graph": 1e3 * t_graph_max / K,
             "ms_per_step_graph_pipelined4": 1e3 * t_graph4_max / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg["name"], "particles": n, "boids": nb, "mc_points_per_axis": G,
-                       "grid_cells": C, "triangles_last_frame": n_tris, "parallelism": "replicas x%d" % world,
-                       "frame_loop": mode + ": the same K frames are timed four ways -- the surface pass of frame t beside "
-                                     "the SPH step of frame t+1 (mc_extract_async), the synchronous calls, the synchronous frame "
-                                     "replayed from a CUDA graph, and a CUDA graph of four pipelined frames -- `value` is the "
-                                     "fastest; `parts` come from the synchronous loop",
-                       "l2": "no explicit flush: the frame's working set (%.0f MB) exceeds the %.0f MB L2 and "
-                             "the state changes every step" % (state_bytes / 1e6, L2_BYTES / 1e6)},
+            "config": workload_config(cfg, world),
+            "run": {"grid_cells": C, "triangles_last_frame": n_tris,
+                    "frame_loop": mode + ": the same K frames are timed four ways -- the surface pass of frame t beside "
+                                  "the SPH step of frame t+1 (mc_extract_async), the synchronous calls, the synchronous frame "
+                                  "replayed from a CUDA graph, and a CUDA graph of four pipelined frames -- `value` is the "
+                                  "fastest; `parts` come from the synchronous loop"},
             "parts": {
                 "sph_boid": {"value": n * K * world / t_sim_max, "unit": "particle-updates/s",
                              "ms_per_step": 1e3 * t_sim_max / K, "algorithmic_gbs": sim_gbs,
