@@ -112,3 +112,21 @@ def test_invalidate_grid_after_rewriting_positions_in_place():
     assert np.array_equal(out["ncount"], ref["ncount"])
     bad, worst = vec_err(out["pos"][:, :3], ref["pos"][:, :3])
     assert bad == 0, (bad, worst)
+
+
+@pytest.mark.parametrize("n,h", [(16384, 1.0 / 20), (16385, 1.0 / 20), (16384, 1.0 / 20.2), (5000, 1.0 / 20.16), (5000, 1.0 / 21)])
+def test_grid_small_and_large_paths_agree_at_their_boundary(n, h):
+    """k_grid_small takes grids of <= 8192 cells and <= 16384 points, the four-kernel path everything else: both sides of
+    either limit (20^3 = 8000 cells, 21^3 = 9261; 16384 / 16385 points), dense cells (a cloud in one corner: ~100 points
+    per cell, the long-run ranking of k_reorder on the large path), against the oracle; and the two paths alternate on one
+    context without disturbing each other (the large path's histogram must still be clear)."""
+    sp = dict(W.config(1)["sph"], h=h)
+    pos = W.random_cloud(n, (0.0, 0.0, 0.0), (0.3, 0.3, 0.25), seed=n)
+    _check(sp, pos)
+    with Sim(dict(sph=sp, n=n)) as sim:
+        rc, rp, rs = R.build_grid(sp, pos)
+        few = pos[:1000].copy()
+        fc, fp, fs = R.build_grid(sp, few)
+        for p_np, want in ((pos, (rc, rp, rs)), (few, (fc, fp, fs)), (pos, (rc, rp, rs))):
+            cell, perm, start = sim.build_grid(dev(p_np), dev(np.zeros_like(p_np)))
+            assert np.array_equal(cell, want[0]) and np.array_equal(perm, want[1]) and np.array_equal(start, want[2])
