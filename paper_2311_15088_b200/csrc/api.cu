@@ -499,8 +499,8 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     launch_force_masks(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS, ctx->rho_bS,
                        (float4*)pos, (float4*)vel, (float4*)accel, touched, (const uint32_t*)ctx->nbr.list, s, &ctx->prof);
   else
-    launch_force_list(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rho_bS, (float4*)pos,
-                      (float4*)vel, (float4*)accel, touched, ctx->nbr, s, &ctx->prof);
+    launch_force_list(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS, ctx->rho_bS,
+                      (float4*)pos, (float4*)vel, (float4*)accel, touched, ctx->nbr, s, &ctx->prof);
   ctx->grid_fresh = false;  // positions moved
   ctx->step_state = true;   // pg / rhoS still describe the step-start state (for boid_step)
   if (n_boid > 0) {

@@ -109,7 +109,7 @@ uint32_t nbr_rows();
 void launch_boid_density(const SphConst& c, const GridBuf& pg, const GridBuf& bg, uint32_t nb, float* rho_bS,
                          cudaStream_t s, Prof* prof);
 void launch_force_list(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
-                       uint32_t nb, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
+                       uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
                        uint32_t* touched_out, const NbrList& nl, cudaStream_t s, Prof* prof);
 // sph_brick.cu: S6 with a brick of cells per block staged in shared memory, S8-S10 from the masks it stores.  masks = one
 // word per target and chunk of 32 candidates, kNbrMaskWords words per sorted particle, row-major.
