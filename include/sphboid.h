@@ -160,7 +160,7 @@ int sph_hashgrid_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, uint3
  * pass stores each particle's neighbour list as 16-bit entries (the paper's section 9 design) and the force
  * pass reads it; 1 = the density pass stages a brick of cells per block in shared memory and stores the neighbour
  * predicate as one bit per candidate, the force pass walks those bits.  Measured on B200: equal at ~8 particles per
- * cell (config 4), 1 is 9 % faster per frame at ~15 per cell (config 5).  Host-side setting, takes effect with the next
+ * cell (config 4), 1 is 12 % faster per frame at ~15 per cell (config 5).  Host-side setting, takes effect with the next
  * sph_step.  Any other value: SPH_E_INVALID. */
 int sph_set_force_variant(sph_ctx* ctx, int variant);
 
