@@ -283,7 +283,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--force-variant", type=int, default=0, help="A/B: 0 = stored neighbour list (default), 1 = brick density pass + neighbour masks")
+    ap.add_argument("--force-variant", type=int, default=0, help="A/B: 0 = cost model (default), 1 = stored neighbour list, 2 = brick density pass + neighbour masks")
     ap.add_argument("--sdf-variant", type=int, default=0, help="A/B: 0 = cost model (default), 1 = per-corner walk, 2 = corner tiles")
     ap.add_argument("--recut-every", type=int, default=0, help="slab decomposition: re-cut the faces by particle count every k frames (0 = never)")
     ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],

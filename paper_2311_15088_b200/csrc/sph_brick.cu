@@ -1,6 +1,6 @@
 // sph_brick.cu -- S6 with the neighbourhood of a BRICK of cells staged once per block in shared memory, and S8-S10 from
 // the neighbour masks it stores.  P:440-471 (Listing 8 + section 9: neighbour search, stored neighbours), P:172 / P:182
-// (density), P:351-375 (Listing 3).  Selected by sph_set_force_variant(ctx, 1); DESIGN.md section 10 has the A/B.
+// (density), P:351-375 (Listing 3).  Selected by sph_set_force_variant(ctx, 2); DESIGN.md section 10 has the A/B.
 //
 //   k_density_brick : a block owns a brick of BX x BY x BZ cells and copies the (BX+2)(BY+2)(BZ+2) cells around it --
 //                     (BY+2)(BZ+2) contiguous x-runs of the cell-sorted positions -- into shared memory once.  A thread

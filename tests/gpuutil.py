@@ -20,7 +20,7 @@ def host_u32(t):
     return t.cpu().numpy().view(np.uint32)
 
 
-FORCE_VARIANT = None  # set by a test fixture: 0 = stored neighbour list, 1 = brick density + neighbour masks (sph_set_force_variant)
+FORCE_VARIANT = None  # set by a test fixture: 1 = stored neighbour list, 2 = brick density + neighbour masks; None = the library's cost model
 
 
 class Sim:
