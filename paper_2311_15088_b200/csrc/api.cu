@@ -463,9 +463,12 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
   if (!(ctx->grid_fresh && ctx->grid_pos == pos && ctx->grid_vel == vel && ctx->grid_n == n))
     build_grid(ctx, pos, vel, n, s);
   ctx->boid_state = false;
-  // 0 = cost model: the mask path pays in dense fluids (measured: equal at ~8 particles per occupied cell, 12 % of the
-  // frame at ~15); the host knows n and the cell count only, so the rule is 'at least 6 particles per cell of the box'
-  const bool brick = ctx->force_variant == 2 || (ctx->force_variant == 0 && (double)n >= 6.0 * (double)ctx->sc.grid.C);
+  // 0 = cost model from what the host knows (n and the cell count).  Measured on B200: the mask path
+  // wins where the passes are throughput-bound -- 1 M particles at ~8 per occupied cell: frame -2.8 %, SPH half -6.6 %;
+  // 4 M at ~15 per cell: frame -12 % -- and loses where they are latency-bound (its density pass launches a block per
+  // brick of the whole grid): 4 K .. 262 K particles, +1 .. +10 % per frame.
+  const bool brick = ctx->force_variant == 2 ||
+                     (ctx->force_variant == 0 && (n >= (1u << 19) || (double)n >= 6.0 * (double)ctx->sc.grid.C));
   if (n_boid > 0) {
     int rc = set_boid_params(ctx, bp);
     if (rc != SPH_OK) return rc;
@@ -484,7 +487,8 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     if (fork) CK(cudaEventRecord(ctx->ev_join, ctx->side));
   }
   if (brick)
-    launch_density_brick(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, (uint32_t*)ctx->nbr.list, s, &ctx->prof);
+    launch_density_brick(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, (uint32_t*)ctx->nbr.list, ctx->nbr.stride, s,
+                         &ctx->prof);
   else
     launch_density(ctx->sc, ctx->pg, n, ctx->rhoS, density, ncount, &ctx->nbr, s, &ctx->prof);
   if (ctx->vel_pending) {  // sph_simulate_host: the velocities arrived on the upload stream while the above ran
@@ -499,7 +503,8 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
   }
   if (brick)
     launch_force_masks(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS, ctx->rho_bS,
-                       (float4*)pos, (float4*)vel, (float4*)accel, touched, (const uint32_t*)ctx->nbr.list, s, &ctx->prof);
+                       (float4*)pos, (float4*)vel, (float4*)accel, touched, (const uint32_t*)ctx->nbr.list,
+                       ctx->nbr.stride, s, &ctx->prof);
   else
     launch_force_list(ctx->sc, n_boid > 0 ? &ctx->bc : nullptr, ctx->pg, ctx->bg, n, n_boid, ctx->rhoS, ctx->rho_bS,
                       (float4*)pos, (float4*)vel, (float4*)accel, touched, ctx->nbr, s, &ctx->prof);

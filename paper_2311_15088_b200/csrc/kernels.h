@@ -112,13 +112,13 @@ void launch_force_list(const SphConst& c, const BoidConst* bc, const GridBuf& pg
                        uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
                        uint32_t* touched_out, const NbrList& nl, cudaStream_t s, Prof* prof);
 // sph_brick.cu: S6 with a brick of cells per block staged in shared memory, S8-S10 from the masks it stores.  masks = one
-// word per target and chunk of 32 candidates, kNbrMaskWords words per sorted particle, row-major.
+// word per target and chunk of 32 candidates, up to kNbrMaskWords words per sorted particle: masks[w * stride + i].
 constexpr int kNbrMaskWords = 32;
 void launch_density_brick(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
-                          uint32_t* ncount_out, uint32_t* masks, cudaStream_t s, Prof* prof);
+                          uint32_t* ncount_out, uint32_t* masks, uint32_t stride, cudaStream_t s, Prof* prof);
 void launch_force_masks(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                         uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
-                        uint32_t* touched_out, const uint32_t* masks, cudaStream_t s, Prof* prof);
+                        uint32_t* touched_out, const uint32_t* masks, uint32_t stride, cudaStream_t s, Prof* prof);
 // boid.cu
 void launch_boid_step(const SphConst& c, const BoidConst& bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                       uint32_t nb, const float* rhoS, const float* rho_bS, float4* bpos, float4* bvel,

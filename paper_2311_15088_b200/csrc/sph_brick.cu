@@ -193,7 +193,7 @@ __device__ __forceinline__ int brick_round(BrickTab& tb, Box& b, const GridDesc&
 // ---- S6 -------------------------------------------------------------------------------------------------------------
 // rho_i = m C6 sum_{r^2 < h^2} (h^2 - r^2)^3, self included; ncount_i = #{r^2 < h^2}; the
 // predicate bits of chunk k (32 candidates from the start of a run, runs in (dz, dy) order) of target i go to
-// masks[i * kNbrMaskWords + w], w counting the target's chunks; candidate j of the chunk is bit 31 - j.
+// masks[w * stride + i], w counting the target's chunks; candidate j of the chunk is bit 31 - j.
 //
 // A thread owns two targets A, B of one cell.  Staged: two candidates per step, loaded as (x0,x1), (y0,y1), (z0,z1);
 // per target three packed subtractions, dist2 and r^2 - h^2 on packed binary32 -- the scalar test's operations in its
@@ -230,7 +230,7 @@ __device__ __forceinline__ void density_box(const SphConst& c, BrickTab& tb, con
                                             const float4* __restrict__ posS, const uint32_t* __restrict__ perm,
                                             float* __restrict__ rhoS, float4* __restrict__ velS,
                                             float* __restrict__ density_out, uint32_t* __restrict__ ncount_out,
-                                            uint32_t* __restrict__ masks) {
+                                            uint32_t* __restrict__ masks, uint32_t stride) {
   const int tid = threadIdx.x;
   const int ny = b.sy + 2;
   const float* sy = sx + cap;
@@ -263,8 +263,10 @@ __device__ __forceinline__ void density_box(const SphConst& c, BrickTab& tb, con
     const f32x2 abx = pack2(pA.x, pB.x), aby = pack2(pA.y, pB.y), abz = pack2(pA.z, pB.z);
     double SA = 0.0, SB = 0.0;
     uint32_t cntA = 0, cntB = 0, w = 0;
-    uint4* mrow = reinterpret_cast<uint4*>(masks + (size_t)iA * kNbrMaskWords);
-    uint4 bufA = make_uint4(0u, 0u, 0u, 0u), bufB = bufA;
+    // word w of target i: masks[w * stride + i]; the lanes' targets are consecutive, so a warp's stores of one word
+    // fall into a few 128-byte lines.  (Tiles of 256 particles, word-major inside a tile -- all words of a particle within
+    // 32 KB -- measured no better at 4 M particles and 3 % worse here: it is not the TLB that the long stride costs.)
+    uint32_t* mcol = masks + iA;
 #pragma unroll 1
     for (int dz = 0; dz < 3; ++dz)
 #pragma unroll 1
@@ -322,16 +324,9 @@ __device__ __forceinline__ void density_box(const SphConst& c, BrickTab& tb, con
 #undef SPHB_TWO
           const uint32_t mA = d.maskA << (32u - nc), mB = d.maskB << (32u - nc);  // candidate j of the chunk -> bit 31 - j
           cntA += __popc(mA), cntB += __popc(mB);
-          const uint32_t wq = w & 3u;
-          if (wq == 0u) bufA.x = mA, bufB.x = mB;
-          if (wq == 1u) bufA.y = mA, bufB.y = mB;
-          if (wq == 2u) bufA.z = mA, bufB.z = mB;
-          if (wq == 3u) {
-            bufA.w = mA, bufB.w = mB;
-            if (w < (uint32_t)kNbrMaskWords) {
-              mrow[w >> 2] = bufA;
-              if (hasB) mrow[(kNbrMaskWords >> 2) + (w >> 2)] = bufB;
-            }
+          if (w < (uint32_t)kNbrMaskWords) {
+            mcol[(size_t)w * stride] = mA;
+            if (hasB) mcol[(size_t)w * stride + 1] = mB;
           }
           ++w;
           float a0, a1, b0, b1, e0, e1;
@@ -340,10 +335,6 @@ __device__ __forceinline__ void density_box(const SphConst& c, BrickTab& tb, con
           SB += (double)((b0 + b1) + e1);
         }
       }
-    if ((w & 3u) != 0u && w < (uint32_t)kNbrMaskWords) {  // the last, partial group of four words
-      mrow[w >> 2] = bufA;
-      if (hasB) mrow[(kNbrMaskWords >> 2) + (w >> 2)] = bufB;
-    }
     const float rhoA = (float)((double)c.mass_c6 * SA), rhoB = (float)((double)c.mass_c6 * SB);
     rhoS[iA] = rhoA;
     reinterpret_cast<float*>(velS + iA)[3] = 1.0f / rhoA;  // the force passes pick 1 / rho_j up with the neighbour's velocity
@@ -370,7 +361,8 @@ __global__ void __launch_bounds__(kDThreads, 8) k_density_brick(SphConst c, cons
                                                              float* __restrict__ rhoS, float4* __restrict__ velS,
                                                              float* __restrict__ density_out,
                                                              uint32_t* __restrict__ ncount_out,
-                                                             uint32_t* __restrict__ masks, uint32_t cap) {
+                                                             uint32_t* __restrict__ masks, uint32_t stride,
+                                                             uint32_t cap) {
   extern __shared__ __align__(16) unsigned char brick_dyn[];
   float* sx = reinterpret_cast<float*>(brick_dyn);
   __shared__ BrickTab tb;
@@ -381,9 +373,9 @@ __global__ void __launch_bounds__(kDThreads, 8) k_density_brick(SphConst c, cons
     if (act == kActDone) break;
     if (act == kActStaged) {
       brick_stage(tb, b, posS, sx, cap);
-      density_box<true>(c, tb, b, sx, cap, posS, perm, rhoS, velS, density_out, ncount_out, masks);
+      density_box<true>(c, tb, b, sx, cap, posS, perm, rhoS, velS, density_out, ncount_out, masks, stride);
     } else if (act == kActGlobal) {
-      density_box<false>(c, tb, b, sx, cap, posS, perm, rhoS, velS, density_out, ncount_out, masks);
+      density_box<false>(c, tb, b, sx, cap, posS, perm, rhoS, velS, density_out, ncount_out, masks, stride);
     }
     block_sync();  // the staged arrays, the tables and the decision are reused by the next round
   }
@@ -405,7 +397,7 @@ constexpr int kMThreads = 128;
 __global__ void __launch_bounds__(kMThreads)
 k_force_masks(SphConst c, BoidConst bc, bool has_boids, const float4* __restrict__ posS,
               const float4* __restrict__ velS, const uint32_t* __restrict__ start, const uint32_t* __restrict__ perm,
-              uint32_t n, const float* __restrict__ rhoS, const uint32_t* __restrict__ masks,
+              uint32_t n, const float* __restrict__ rhoS, const uint32_t* __restrict__ masks, uint32_t stride,
               const float4* __restrict__ bposS, const float4* __restrict__ bvelS, const float* __restrict__ rho_bS,
               const uint32_t* __restrict__ bstart, float4* __restrict__ pos, float4* __restrict__ vel,
               float4* __restrict__ accel_out, uint32_t* __restrict__ touched_out) {
@@ -445,8 +437,10 @@ k_force_masks(SphConst c, BoidConst bc, bool has_boids, const float4* __restrict
     }
     ne = 0;
   };
-  const uint4* mrow = reinterpret_cast<const uint4*>(masks + (size_t)i * kNbrMaskWords);
-  uint4 cur = __ldg(mrow), nxt = __ldg(mrow + 1);
+  // word w: mcol[w * stride], one coalesced load per warp; fetched four words ahead (the rows live in L2 / HBM)
+  const uint32_t* mcol = masks + i;
+  uint32_t q0 = __ldg(mcol), q1 = __ldg(mcol + stride), q2 = __ldg(mcol + 2u * (size_t)stride),
+           q3 = __ldg(mcol + 3u * (size_t)stride);
   uint32_t w = 0;
   bool overflow = false;
 #pragma unroll 1
@@ -459,13 +453,10 @@ k_force_masks(SphConst c, BoidConst bc, bool has_boids, const float4* __restrict
         overflow = true;
         break;
       }
-      const uint32_t sel = w & 3u;
-      const uint32_t m = sel == 0u ? cur.x : (sel == 1u ? cur.y : (sel == 2u ? cur.z : cur.w));
+      const uint32_t m = q0;
+      q0 = q1, q1 = q2, q2 = q3;
       ++w;
-      if ((w & 3u) == 0u) {  // the next four words were fetched while these were looked at
-        cur = nxt;
-        if (w + 4u < (uint32_t)kNbrMaskWords) nxt = __ldg(mrow + (w >> 2) + 1);
-      }
+      if (w + 3u < (uint32_t)kNbrMaskWords) q3 = __ldg(mcol + (size_t)(w + 3u) * stride);
       if (m != 0u) {
         tabm[ne * kMThreads] = m;
         tabb[ne * kMThreads] = c0;
@@ -494,24 +485,24 @@ uint32_t brick_blocks(const GridDesc& g) {
 // box that exceeds the capacity is split, so the choice only moves where the split happens.
 constexpr uint32_t kBrickCap = 2048;   // k_density_brick: 24 KB of x / y / z
 void launch_density_brick(const SphConst& c, const GridBuf& b, uint32_t n, float* rhoS, float* density_out,
-                          uint32_t* ncount_out, uint32_t* masks, cudaStream_t s, Prof* prof) {
+                          uint32_t* ncount_out, uint32_t* masks, uint32_t stride, cudaStream_t s, Prof* prof) {
   if (n == 0) return;
   const size_t smem = (size_t)kBrickCap * 12;
   prof->begin(K_DENSITY_BRICK, s);
   k_density_brick<<<brick_blocks(c.grid), kDThreads, smem, s>>>(c, b.posS, b.start, b.perm, rhoS, b.velS, density_out,
-                                                                ncount_out, masks, kBrickCap);
+                                                                ncount_out, masks, stride, kBrickCap);
   prof->end(s);
 }
 
 void launch_force_masks(const SphConst& c, const BoidConst* bc, const GridBuf& pg, const GridBuf& bg, uint32_t n,
                         uint32_t nb, const float* rhoS, const float* rho_bS, float4* pos, float4* vel, float4* accel_out,
-                        uint32_t* touched_out, const uint32_t* masks, cudaStream_t s, Prof* prof) {
+                        uint32_t* touched_out, const uint32_t* masks, uint32_t stride, cudaStream_t s, Prof* prof) {
   if (n == 0) return;
   BoidConst dummy = {};
   const bool has = nb > 0 && bc != nullptr;
   prof->begin(K_FORCE_MASKS, s);
   k_force_masks<<<(n + kMThreads - 1) / kMThreads, kMThreads, 0, s>>>(
-      c, has ? *bc : dummy, has, pg.posS, pg.velS, pg.start, pg.perm, n, rhoS, masks, bg.posS, bg.velS, rho_bS,
+      c, has ? *bc : dummy, has, pg.posS, pg.velS, pg.start, pg.perm, n, rhoS, masks, stride, bg.posS, bg.velS, rho_bS,
       bg.start, pos, vel, accel_out, touched_out);
   prof->end(s);
 }
