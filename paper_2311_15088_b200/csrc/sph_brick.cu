@@ -417,23 +417,33 @@ k_force_masks(SphConst c, BoidConst bc, bool has_boids, const float4* __restrict
   uint32_t ne = 0;
   auto consume = [&]() {
     uint32_t e = 0, m = 0, base = 0;
-#pragma unroll 1
-    for (;;) {
+    // next two set bits of the stream -> slots; false when the stream is exhausted.  An odd count leaves the second
+    // half on the target itself: r^2 = 0, no force
+    auto pop2 = [&](uint32_t& sl0, uint32_t& sl1) -> bool {
+      sl0 = sl1 = i;
       if (m == 0u) {
-        if (e == ne) break;
+        if (e == ne) return false;
         m = tabm[e * kMThreads], base = tabb[e * kMThreads], ++e;
       }
       uint32_t j = __clz(m);
       m ^= 0x80000000u >> j;
-      const uint32_t sl0 = base + j;
-      uint32_t sl1 = i;  // odd count: the second half reads the target itself, r^2 = 0, no force
+      sl0 = base + j;
       if (m == 0u && e != ne) m = tabm[e * kMThreads], base = tabb[e * kMThreads], ++e;
       if (m != 0u) {
         j = __clz(m);
         m ^= 0x80000000u >> j;
         sl1 = base + j;
       }
-      eval_two(kf2, __ldg(posS + sl0), __ldg(velS + sl0), __ldg(posS + sl1), __ldg(velS + sl1), pi, vi, rho_m, F);
+      return true;
+    };
+    uint32_t a0, a1;
+    bool more = pop2(a0, a1);
+#pragma unroll 1
+    while (more) {
+      // the gathers of this pair are issued, then the next pair's slots are popped while they are in flight
+      const float4 p0 = __ldg(posS + a0), v0 = __ldg(velS + a0), p1 = __ldg(posS + a1), v1 = __ldg(velS + a1);
+      more = pop2(a0, a1);
+      eval_two(kf2, p0, v0, p1, v1, pi, vi, rho_m, F);
     }
     ne = 0;
   };
