@@ -159,8 +159,8 @@ int sph_hashgrid_neighbor_count(sph_ctx* ctx, const void* pos, uint32_t n, uint3
 /* S6 / S8 exist twice, computing the same densities and forces (DESIGN.md sections 6 and 10): 1 = the density pass
  * stores each particle's neighbour list as 16-bit entries (the paper's section 9 design) and the force pass
  * reads it; 2 = the density pass stages a brick of cells per block in shared memory and stores the neighbour predicate
- * as one bit per candidate, the force pass walks those bits.  Measured on B200, whole frame: 2 is 2.8 % faster at 1 M
- * particles (config 4), 12 % at 4 M compressed ones (config 5), 1 is 1-10 % faster at 4 K - 262 K (configs 1-3, where
+ * as one bit per candidate, the force pass walks those bits.  Measured on B200, whole frame: 2 is 3 % faster at 1 M
+ * particles (config 4), 14 % at 4 M compressed ones (config 5), 1 is 1-10 % faster at 4 K - 262 K (configs 1-3, where
  * the passes are latency-bound).  0 (default) picks by a cost model: 2 when n >= 2^19 or the box holds at least 6
  * particles per grid cell on average (n >= 6 C), else 1.  Host-side setting, takes effect with the next
  * sph_step.  Any other value: SPH_E_INVALID. */

@@ -464,8 +464,8 @@ int sph_step(sph_ctx* ctx, void* pos, void* vel, uint32_t n, const void* bpos, c
     build_grid(ctx, pos, vel, n, s);
   ctx->boid_state = false;
   // 0 = cost model from what the host knows (n and the cell count).  Measured on B200: the mask path
-  // wins where the passes are throughput-bound -- 1 M particles at ~8 per occupied cell: frame -2.8 %, SPH half -6.6 %;
-  // 4 M at ~15 per cell: frame -12 % -- and loses where they are latency-bound (its density pass launches a block per
+  // wins where the passes are throughput-bound -- 1 M particles at ~8 per occupied cell: frame -3 %, SPH half -8 %;
+  // 4 M at ~15 per cell: frame -14 % -- and loses where they are latency-bound (its density pass launches a block per
   // brick of the whole grid): 4 K .. 262 K particles, +1 .. +10 % per frame.
   const bool brick = ctx->force_variant == 2 ||
                      (ctx->force_variant == 0 && (n >= (1u << 19) || (double)n >= 6.0 * (double)ctx->sc.grid.C));
