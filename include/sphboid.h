@@ -259,6 +259,28 @@ int sph_profile_enable(sph_ctx* ctx, int enable);
 int sph_profile_read(sph_ctx* ctx, uint32_t kernel_id, uint64_t* launches_host, double* total_ms_host);
 const char* sph_kernel_name(uint32_t kernel_id);
 
+/* ---- An entry point that allocates nothing -----------------------------------------------------------------------------
+ * sph_build_grid_static: S1-S5 without a context -- for callers that may not call
+ * cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  It calls no cudaMalloc,
+ * cudaFree or allocating library routine, on its first call or any later one; its scratch (the key and the arrival rank
+ * of every point) is a file-scope __device__ array of 2 x SPH_STATIC_MAX_POINTS x 4 B = 128 KB that every GPU which
+ * loads the library holds until the process exits.  Runs on the CURRENT device, asynchronously on `stream`.
+ *   box_min, box_max (host, 3 floats each), h: the grid of sph_create with these values (D:A-DIMS); C = its cell count.
+ *   pos (device, n x float4, 16-byte aligned): the points; .w ignored.
+ *   cell_of_particle[n], perm[n] (sorted slot -> id, ascending id inside a cell), cell_start[C + 1] (device, all
+ *   required, caller-owned): the same values sph_build_grid returns, bit for bit.  cell_start_entries = the number of
+ *   entries cell_start can hold (>= C + 1, else SPH_E_INVALID).
+ * Limits: n <= SPH_STATIC_MAX_POINTS and C <= SPH_STATIC_MAX_CELLS, else SPH_E_CAPACITY and nothing is launched.
+ * The scratch is shared by every call on a device and keeps the last call's contents (nothing in it needs clearing: every
+ * word a call reads it has written first); calls that overlap on one GPU -- two streams, two host threads -- race on it.
+ * Errors: sph_status as elsewhere; the message of the calling thread's last failure is sph_static_last_error(). */
+#define SPH_STATIC_MAX_POINTS 16384u
+#define SPH_STATIC_MAX_CELLS 8192u
+int sph_build_grid_static(const float* box_min, const float* box_max, float h, const void* pos, uint32_t n,
+                          void* stream, uint32_t* cell_of_particle, uint32_t* perm, uint32_t* cell_start,
+                          uint32_t cell_start_entries);
+const char* sph_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

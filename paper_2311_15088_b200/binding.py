@@ -104,13 +104,16 @@ def lib():
         L.sph_profile_read.argtypes = [_vp, _u32, _vp, _vp]
         L.sph_kernel_name.argtypes = [_u32]
         L.sph_kernel_name.restype = C.c_char_p
+        L.sph_build_grid_static.argtypes = [_vp, _vp, _f, _vp, _u32, _vp, _vp, _vp, _vp, _u32]
+        L.sph_static_last_error.argtypes = []
+        L.sph_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_last_error", "sph_grid_dims", "sph_build_grid", "sph_step", "boid_step",
            "sph_particle_aabb", "sph_invalidate_grid", "mc_voxel_sdf", "mc_set_sdf_variant", "mc_set_cube_range", "sph_set_force_variant", "boid_set_obstacles", "sph_neighbor_count", "sph_pack_range", "sph_hashgrid_neighbor_count", "mc_polygonise", "mc_extract", "mc_extract_async", "mc_wait", "mc_polygonise_indexed", "mc_extract_indexed", "mc_mesh_components", "sph_simulate_host", "sph_mc_table", "sph_launch_count", "sph_profile_enable",
-           "sph_profile_read", "sph_kernel_name"]
+           "sph_profile_read", "sph_kernel_name", "sph_build_grid_static", "sph_static_last_error"]
 
 
 def _ptr(t):
@@ -203,6 +206,22 @@ def sph_build_grid(ctx, pos, vel=None, stream=None, cell_of_particle=None, perm=
     n = 0 if pos is None else pos.shape[0]
     return _check(ctx, lib().sph_build_grid(ctx, _ptr(pos), _ptr(vel), n, _stream(stream), _ptr(cell_of_particle),
                                             _ptr(perm), _ptr(cell_start)))
+
+
+SPH_STATIC_MAX_POINTS, SPH_STATIC_MAX_CELLS = 16384, 8192
+
+
+def sph_build_grid_static(box_min, box_max, h, pos, cell_of_particle, perm, cell_start, stream=None):
+    """S1-S5 without a context and without any allocation (include/sphboid.h): at most SPH_STATIC_MAX_POINTS points and
+    SPH_STATIC_MAX_CELLS cells; the outputs are the caller's CUDA tensors (cell_start: at least C + 1 entries)."""
+    lo = (_f * 3)(*[float(v) for v in box_min])
+    hi = (_f * 3)(*[float(v) for v in box_max])
+    n = 0 if pos is None else pos.shape[0]
+    rc = lib().sph_build_grid_static(lo, hi, float(h), _ptr(pos), n, _stream(stream), _ptr(cell_of_particle), _ptr(perm),
+                                     _ptr(cell_start), 0 if cell_start is None else cell_start.numel())
+    if rc != SPH_OK:
+        raise SphError(rc, lib().sph_static_last_error().decode())
+    return rc
 
 
 def sph_step(ctx, pos, vel, bpos=None, bvel=None, boid=None, stream=None, density=None, accel=None, ncount=None,

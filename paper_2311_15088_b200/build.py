@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libsphboid.so")
-SOURCES = ["api.cu", "grid.cu", "sph.cu", "sph_brick.cu", "boid.cu", "mc.cu"]
+SOURCES = ["api.cu", "grid.cu", "sph.cu", "sph_brick.cu", "boid.cu", "mc.cu", "noalloc.cu"]
 HEADERS = ["common.cuh", "kernels.h", "sph_common.cuh", "mc_table.inc"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--fmad=true",

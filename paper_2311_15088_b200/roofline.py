@@ -122,14 +122,15 @@ def alu_point(kernel, avg_us, pairs, sm_mhz):
 
 
 def csrc_sha16():
-    """Hash of the CUDA sources that hold the kernels (everything under csrc/ except api.cu, which is host-side glue):
-    stamps profiles/traffic.csv, so that bench.py only quotes a DRAM-traffic figure captured on the kernels it is timing."""
+    """Hash of the CUDA sources that hold the frame's kernels (everything under csrc/ except api.cu, which is host-side
+    glue, and noalloc.cu, whose one kernel bench.py never launches): stamps profiles/traffic.csv, so that bench.py only
+    quotes a DRAM-traffic figure captured on the kernels it is timing."""
     import hashlib
     import os
     d = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc")
     h = hashlib.sha256()
     for name in sorted(os.listdir(d)):
-        if name.endswith((".cu", ".cuh", ".h", ".inc")) and name != "api.cu":
+        if name.endswith((".cu", ".cuh", ".h", ".inc")) and name not in ("api.cu", "noalloc.cu"):
             h.update(name.encode())
             h.update(open(os.path.join(d, name), "rb").read())
     return h.hexdigest()[:16]
