@@ -69,11 +69,14 @@ def test_static_grid_build_takes_no_device_memory_after_its_first_call():
     C = 16 ** 3
     pos_t, cell_t, perm_t, start_t = dev(pos), u32(pos.shape[0]), u32(pos.shape[0]), u32(C + 1)
     _static(sp, pos_t, cell_t, perm_t, start_t)  # the first launch may load the kernel's module
-    free0, _ = torch.cuda.mem_get_info()
-    for _ in range(3):
-        _static(sp, pos_t, cell_t, perm_t, start_t)
-    free1, _ = torch.cuda.mem_get_info()
-    assert free1 == free0
+    same = False
+    for attempt in range(3):  # the figure is device-wide: another process may move it once, not three times in a row
+        free0, _ = torch.cuda.mem_get_info()
+        for _ in range(3):
+            _static(sp, pos_t, cell_t, perm_t, start_t)
+        free1, _ = torch.cuda.mem_get_info()
+        same = same or free1 == free0
+    assert same
 
 
 def test_static_grid_build_rejects_sizes_beyond_its_maximum_and_bad_arguments():
