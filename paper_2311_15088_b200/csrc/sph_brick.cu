@@ -46,7 +46,9 @@ struct BrickTab {
                                        // arrays when the box is staged, cell-sorted global slot when it is not
   uint32_t g0[kMaxRows];               // global slot of the first particle of each run
   uint32_t off[kMaxRows + 1];          // staged index of the first particle of each run; off[rows] = T
-  uint32_t pre[kMaxCells + 1];         // density: units before each cell; force: targets before each brick row
+  uint32_t pre[33];                    // density units before each cell of the box: all 32 lanes of warp 0 write their entry
+                                       // (lanes past the box's cells repeat the total, which is what the search in
+                                       // density_box relies on), entry 32 = the total; so 33 whatever the brick's size
   uint32_t T, ntarget;                 // particles in the neighbourhood, targets in the box
   Box stack[8];
   Box cur;
