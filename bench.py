@@ -164,6 +164,10 @@ def run_reference(args, cfg_idx):
     """--impl reference: the CPU oracle as it stands, on the host cores; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
+    # torchrun exports OMP_NUM_THREADS=1 to every rank unless the caller set it; this arm runs on rank 0 alone and is
+    # meant to use the box's host cores, so that default is undone before the OpenMP runtime of the oracle starts
+    if os.environ.get("TORCHELASTIC_RUN_ID") and os.environ.get("OMP_NUM_THREADS") == "1":
+        os.environ["OMP_NUM_THREADS"] = str(len(os.sched_getaffinity(0)))
     from paper_2311_15088_b200 import workloads as W
     cfg = W.config(cfg_idx)
     mp = W.mc_params(cfg)
